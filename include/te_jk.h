@@ -1,0 +1,112 @@
+/*
+ * te_jk.h -- C ABI of the B200-native direct-SCF Coulomb/exchange (J/K) Fock build.
+ *
+ * Method: arXiv 2406.14920 (PAPER.md; "P:n" = line n).  Four-centre electron-repulsion integrals over
+ * contracted Cartesian Gaussian shells l = 0..3 (eq. 27-31), McMurchie-Davidson scheme
+ * (E eq. 5-8, Boys eq. 18, R eq. 20-25), contracted on the fly with a density matrix into
+ *   J_mu,nu     = sum_{lambda,sigma} (mu nu|lambda sigma) D_lambda,sigma      (eq. 34)
+ *   K_mu,lambda = sum_{nu,sigma}     (mu nu|lambda sigma) D_nu,sigma          (eq. 36)
+ * over Schwarz-screened PRIMITIVE shell pairs (eq. 45) with the per-term density-weighted
+ * test of eq. 47.  No factors of 2 or 1/2 are applied to J or K.
+ *
+ * Conventions
+ *  - Every function returns TE_OK (0) or a negative TE_ERR_* code; te_last_error() gives a thread-local
+ *    message.  No C++ exception and no exit() crosses this boundary.
+ *  - "host" / "device" says where a pointer must live.  Handles (te_basis, te_pairs) are library-owned:
+ *    create with te_*_create / te_shellpair_build, free with te_*_destroy.  All other buffers are
+ *    caller-owned.
+ *  - Lengths in bohr.  Matrices are row-major nbf x nbf FP64.  AO order = caller's shell order; inside a
+ *    shell the Cartesian components are lexicographic with x^l first:
+ *      p: x y z;  d: xx xy xz yy yz zz;  f: xxx xxy xxz xyy xyz xzz yyy yyz yzz zzz.
+ *  - Every contracted Cartesian function is normalised to unit self-overlap (eq. 1-2); the
+ *    caller passes RAW contraction coefficients.
+ *  - There is no CPU fallback: every call that computes needs a CUDA device (sm_100a build).
+ */
+#ifndef TE_JK_H
+#define TE_JK_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TE_OK 0
+#define TE_ERR_BAD_ARG (-1)
+#define TE_ERR_UNSUPPORTED_L (-2)
+#define TE_ERR_ALLOC (-3)
+#define TE_ERR_CUDA (-4)
+
+#define TE_NCLASS 10 /* primitive shell-pair classes SS SP SD SF PP PD PF DD DF FF */
+
+typedef struct te_basis te_basis; /* opaque */
+typedef struct te_pairs te_pairs; /* opaque */
+
+/* Basis (eq. 1-2).  All pointers HOST.  xyz_bohr[natoms][3]; shell_atom/shell_l/shell_nprim
+ * [nshells]; exponents/coefficients concatenated over shells in shell order (sum of shell_nprim entries).
+ * l > 3 -> TE_ERR_UNSUPPORTED_L.  Normalises, uploads to the current CUDA device, returns a handle. */
+int te_basis_create(int natoms, const double *xyz_bohr, int nshells, const int *shell_atom,
+                    const int *shell_l, const int *shell_nprim, const double *exponents,
+                    const double *coefficients, te_basis **out);
+void te_basis_destroy(te_basis *b);
+/* Number of Cartesian basis functions, sum of (l+1)(l+2)/2. */
+int te_basis_nbf(const te_basis *b);
+/* Number of primitive shells, sum of shell_nprim. */
+int te_basis_nprim(const te_basis *b);
+/* offsets[nshells+1] HOST: first AO of every shell. */
+int te_basis_shell_offsets(const te_basis *b, int *offsets);
+/* norm[nprim] HOST: normalised primitive coefficient c~ (x^l component) of every primitive shell. */
+int te_basis_norm_coefs(const te_basis *b, double *norm);
+
+/* Primitive shell-pair lists (section 3.2): all unordered primitive shell pairs, Schwarz bound
+ * q = max over components of sqrt|(mu nu|mu nu)| (eq. 45), pairs with q < pair_threshold (PQTHRE)
+ * dropped, survivors binned into the 10 (la<=lb) classes and sorted by q descending inside each class.
+ * Computed on the device.  pair_threshold = 0 keeps every pair. */
+int te_shellpair_build(const te_basis *b, double pair_threshold, te_pairs **out);
+void te_pairs_destroy(te_pairs *p);
+/* class_count[10], *nkept: HOST outputs. */
+int te_pairs_info(const te_pairs *p, long long class_count[TE_NCLASS], long long *nkept);
+/* HOST copies of class `cls` in the library's sorted order (arrays of class_count[cls] entries; any pointer
+ * may be NULL): contracted shell ids, primitive index inside each shell, Schwarz bound. */
+int te_pairs_export(const te_pairs *p, int cls, int *shellA, int *shellB, int *primA, int *primB,
+                    double *bound);
+/* HOST copies: Gaussian product centre P [n][3], exponent p = a+b, and prefactor
+ * c~_m c~_n exp(-ab/p |A-B|^2) (eq. 3). */
+int te_pairs_export_geom(const te_pairs *p, int cls, double *P_xyz, double *p_exp, double *prefactor);
+
+/* One J/K build (section 3.4).  D_dev, J_dev, K_dev: DEVICE, row-major nbf x nbf; D must be
+ * symmetric; J and K are OVERWRITTEN (not accumulated) and returned symmetric.  threshold = THRECL of
+ * eq. 47; 0 means no screening.  A primitive quartet's contribution X <- D_YZ is included iff
+ * q_bra * q_ket * max|D_YZ block| >= threshold, separately for each of its J and K updates.
+ * Asynchronous on cuda_stream (a cudaStream_t, NULL = default stream). */
+int te_build_jk(const te_pairs *p, const double *D_dev, double *J_dev, double *K_dev, double threshold,
+                void *cuda_stream);
+/* Same build with HOST D, J, K (pinned or pageable): copies in, builds, copies out, synchronises. */
+int te_build_jk_host(const te_pairs *p, const double *D_host, double *J_host, double *K_host,
+                     double threshold);
+/* Statistics of the LAST te_build_jk on this handle (synchronises the build's stream).  HOST outputs,
+ * indexed [bra class][ket class] (only bra class <= ket class is used): unique primitive quartets that
+ * had at least one live update, and device milliseconds spent in that class pair's kernel. */
+int te_jk_stats(const te_pairs *p, long long quartets[TE_NCLASS][TE_NCLASS], float ms[TE_NCLASS][TE_NCLASS]);
+/* Enable (1) / disable (0) per-class CUDA-event timing for te_jk_stats (off by default). */
+int te_jk_set_profiling(te_pairs *p, int on);
+
+/* Contracted, normalised integral blocks for testing (eq. 30).  quartets[n][4] HOST shell ids (A,B,C,D);
+ * out_offsets[n+1] HOST; out_dev DEVICE with out_offsets[n] doubles:
+ *   out_dev[out_offsets[q] + ((i*nB + j)*nC + k)*nD + l] = (A_i B_j | C_k D_l).  No screening. */
+int te_eri_block(const te_basis *b, int nquartets, const int *quartets, const long long *out_offsets,
+                 double *out_dev);
+
+/* Boys function F_0..F_mmax(T) (eq. 18) evaluated by the device routine the kernels use
+ * (tabulated Taylor expansion + downward recursion; asymptotic form + upward recursion for large T).
+ * T_dev[n] DEVICE in; F_dev[n][mmax+1] DEVICE out; mmax <= 12. */
+int te_boys(int n, const double *T_dev, int mmax, double *F_dev);
+
+/* Sustained FP64 FMA throughput of the device (register-resident DFMA chains), in TFLOP/s: the measured
+ * denominator of the "alu" roofline. */
+int te_measure_fp64_peak(double *tflops);
+
+const char *te_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TE_JK_H */

@@ -1,0 +1,63 @@
+"""Build paper_2406_14920_b200/libte_jk.so (C ABI of include/te_jk.h) with nvcc for sm_100a, in-tree.
+
+The per-class kernels are compiled as 10 translation units (te_inst.cu with -DTE_CB=0..9) in parallel.
+Objects are cached under paper_2406_14920_b200/build/ and rebuilt when any source is newer.
+"""
+from __future__ import annotations
+
+import concurrent.futures as cf
+import glob
+import os
+import shutil
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+BUILD = os.path.join(HERE, "build")
+LIB = os.path.join(HERE, "libte_jk.so")
+NVCC = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC",
+         "-Xptxas", "-v", "--expt-relaxed-constexpr"]
+
+
+def _deps_mtime() -> float:
+    files = glob.glob(os.path.join(CSRC, "*")) + [os.path.join(HERE, "..", "include", "te_jk.h")]
+    return max(os.path.getmtime(f) for f in files)
+
+
+def _compile(job):
+    src, obj, extra = job
+    log = obj + ".log"
+    cmd = [NVCC] + FLAGS + extra + ["-c", src, "-o", obj]
+    with open(log, "w") as fh:
+        fh.write(" ".join(cmd) + "\n")
+        fh.flush()
+        r = subprocess.run(cmd, stdout=fh, stderr=subprocess.STDOUT)
+    if r.returncode != 0:
+        raise RuntimeError(f"nvcc failed for {obj}:\n" + open(log).read()[-4000:])
+    return obj
+
+
+def build(force: bool = False, jobs: int | None = None) -> str:
+    newest = _deps_mtime()
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
+        return LIB
+    os.makedirs(BUILD, exist_ok=True)
+    work = [(os.path.join(CSRC, "te_lib.cu"), os.path.join(BUILD, "te_lib.o"), []),
+            (os.path.join(CSRC, "te_dispatch.cu"), os.path.join(BUILD, "te_dispatch.o"), [])]
+    # heaviest bra classes first so the pool stays busy
+    for cb in (9, 8, 7, 6, 5, 4, 3, 2, 1, 0):
+        work.append((os.path.join(CSRC, "te_inst.cu"), os.path.join(BUILD, f"te_inst_{cb}.o"), [f"-DTE_CB={cb}"]))
+    todo = [w for w in work if force or not os.path.exists(w[1]) or os.path.getmtime(w[1]) < newest]
+    with cf.ThreadPoolExecutor(max_workers=jobs or min(12, os.cpu_count() or 4)) as ex:
+        list(ex.map(_compile, todo))
+    objs = [w[1] for w in work]
+    cmd = [NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB + ".tmp"] + objs
+    subprocess.run(cmd, check=True)
+    os.replace(LIB + ".tmp", LIB)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv))

@@ -1,0 +1,89 @@
+// te_inst.cu -- instantiates every kernel whose BRA pair class is TE_CB (compiled 10 times, -DTE_CB=0..9, so the
+// 55 (la lb|lc ld) classes build in parallel).  Exposes launch_*_cb<TE_CB> entry points used by te_dispatch.cu.
+#include "te_kernels.cuh"
+
+#ifndef TE_CB
+#error "compile with -DTE_CB=<bra class 0..9>"
+#endif
+
+namespace te {
+
+constexpr int CLS_LA[TE_NCLASS] = {0, 0, 0, 0, 1, 1, 1, 2, 2, 3};
+constexpr int CLS_LB[TE_NCLASS] = {0, 1, 2, 3, 1, 2, 3, 2, 3, 3};
+constexpr int LA = CLS_LA[TE_CB], LB = CLS_LB[TE_CB];
+
+static BasisView view(const te_basis* b) { return BasisView{b->d_exp, b->d_ct, b->d_xyz, b->d_shell, b->d_off}; }
+
+#define TE_CAT2(a, b) a##b
+#define TE_CAT(a, b) TE_CAT2(a, b)
+
+int TE_CAT(launch_schwarz_cb, TE_CB)(const te_basis* b, long long ncand, double* d_q, long long* d_idx) {
+    const long long nb = b->l_start[LB + 1] - b->l_start[LB];
+    const unsigned grid = (unsigned)((ncand + 63) / 64);
+    schwarz_kernel<LA, LB><<<grid, 64>>>(view(b), b->d_by_l + b->l_start[LA], b->d_by_l + b->l_start[LB], nb, ncand, b->d_boys, d_q, d_idx);
+    TE_CUDA(cudaGetLastError());
+    return TE_OK;
+}
+
+int TE_CAT(launch_pair_fill_cb, TE_CB)(const te_basis* b, long long n, const long long* d_idx, PairD* d_pair, PairIds* d_ids) {
+    const long long nb = b->l_start[LB + 1] - b->l_start[LB];
+    pair_fill_kernel<LA, LB><<<(unsigned)((n + 127) / 128), 128>>>(view(b), b->d_by_l + b->l_start[LA], b->d_by_l + b->l_start[LB], nb, n, d_idx, d_pair, d_ids);
+    TE_CUDA(cudaGetLastError());
+    return TE_OK;
+}
+
+template <int CK>
+static int jk_launch(te_pairs* P, double tau, cudaStream_t st) {
+    constexpr int LC = CLS_LA[CK], LD = CLS_LB[CK];
+    constexpr bool light = use_full_unroll(LA, LB, LC, LD);
+    constexpr int TB = light ? 16 : 8, TK = light ? 16 : 8;
+    const te_basis* b = P->basis;
+    const int slot = TE_CB * TE_NCLASS + CK;
+    JKArgs a;
+    a.pb = P->d_pair[TE_CB]; a.qb = P->d_q[TE_CB]; a.ib = P->d_ids[TE_CB]; a.nb = P->count[TE_CB];
+    a.pk = P->d_pair[CK]; a.qk = P->d_q[CK]; a.ik = P->d_ids[CK]; a.nk = P->count[CK];
+    a.Ds = P->d_Ds; a.Dm = P->d_Dm; a.Jt = P->d_Jt; a.Kt = P->d_Kt; a.boys_tab = b->d_boys;
+    a.tile_start = P->d_tile_start; a.ctrl = P->d_ctrl; a.tau = tau; a.nbf = b->nbf; a.nshells = b->nshells;
+    a.slot = slot; a.same = (TE_CB == CK);
+    schedule_kernel<<<1, 1024, 0, st>>>(a.qb, a.nb, a.qk, a.nk, a.same, tau, TB, TK, P->d_tile_start, P->d_ctrl, slot);
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const long long max_tiles = ((a.nb + TB - 1) / TB) * ((a.nk + TK - 1) / TK);
+    const int per_sm = light ? 8 : 16;   // resident CTAs per SM worth of persistent blocks
+    const unsigned grid = (unsigned)std::min<long long>(max_tiles, (long long)sms * per_sm);
+    jk_kernel<LA, LB, LC, LD, TB, TK><<<grid, TB * TK, 0, st>>>(a);
+    TE_CUDA(cudaGetLastError());
+    return TE_OK;
+}
+
+template <int CK>
+static int eri_launch(const te_basis* b, int n, const EriTask* d_tasks, double* out_dev) {
+    constexpr int LC = CLS_LA[CK], LD = CLS_LB[CK];
+    eri_block_kernel<LA, LB, LC, LD><<<(n + 31) / 32, 32>>>(view(b), b->d_shell_pstart, n, d_tasks, b->d_boys, out_dev);
+    TE_CUDA(cudaGetLastError());
+    return TE_OK;
+}
+
+template <int CK>
+static int jk_dispatch(int ck, te_pairs* P, double tau, cudaStream_t st) {
+    if (ck == CK) return jk_launch<CK>(P, tau, st);
+    if constexpr (CK + 1 < TE_NCLASS) return jk_dispatch<CK + 1>(ck, P, tau, st);
+    set_error("launch_jk: bad ket class %d", ck);
+    return TE_ERR_BAD_ARG;
+}
+
+template <int CK>
+static int eri_dispatch(int ck, const te_basis* b, int n, const EriTask* d_tasks, double* out_dev) {
+    if (ck == CK) return eri_launch<CK>(b, n, d_tasks, out_dev);
+    if constexpr (CK + 1 < TE_NCLASS) return eri_dispatch<CK + 1>(ck, b, n, d_tasks, out_dev);
+    set_error("launch_eri: bad ket class %d", ck);
+    return TE_ERR_BAD_ARG;
+}
+
+int TE_CAT(launch_jk_cb, TE_CB)(int ck, te_pairs* P, double tau, cudaStream_t st) { return jk_dispatch<TE_CB>(ck, P, tau, st); }
+int TE_CAT(launch_eri_cb, TE_CB)(int ck, const te_basis* b, int n, const EriTask* d_tasks, double* out_dev) {
+    return eri_dispatch<TE_CB>(ck, b, n, d_tasks, out_dev);
+}
+
+}  // namespace te

@@ -1,0 +1,80 @@
+// te_internal.h -- handle layouts and launch prototypes shared by the translation units of libte_jk.so.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <vector>
+
+#include "../../include/te_jk.h"
+#include "te_md.cuh"
+
+namespace te {
+
+void set_error(const char* fmt, ...);
+
+#define TE_CUDA(expr)                                                                      \
+    do {                                                                                   \
+        cudaError_t e__ = (expr);                                                          \
+        if (e__ != cudaSuccess) {                                                          \
+            te::set_error("%s:%d: %s: %s", __FILE__, __LINE__, #expr, cudaGetErrorString(e__)); \
+            return TE_ERR_CUDA;                                                            \
+        }                                                                                  \
+    } while (0)
+
+struct PairIds {
+    int m, n;        // global primitive-shell ids, (l_m, m) <= (l_n, n)
+    int shA, shB;    // contracted shell ids
+    int offA, offB;  // first AO of each contracted shell
+};
+
+struct JKControl {
+    double dmax;                                        // max |D| (set by density_bounds_kernel)
+    unsigned long long live[TE_NCLASS * TE_NCLASS];     // unique live quartets per class pair
+    unsigned long long ntiles[TE_NCLASS * TE_NCLASS];   // scheduled tiles per class pair
+    unsigned int tile_counter[TE_NCLASS * TE_NCLASS];   // dynamic tile queue heads
+};
+
+struct EriTask {
+    int sh[4];       // canonical order: la<=lb, lc<=ld, class(ab)<=class(cd)
+    int stride[4];   // output stride of each canonical index
+    long long out;   // offset of the block in out_dev
+};
+
+}  // namespace te
+
+struct te_basis {
+    int natoms = 0, nshells = 0, nprim = 0, nbf = 0;
+    std::vector<int> shell_l, shell_off, shell_pstart, shell_nprim;
+    std::vector<double> prim_exp, prim_ct, prim_xyz;
+    std::vector<int> prim_l, prim_shell, prim_iprim, prim_off, prims_by_l;
+    int l_start[5] = {0, 0, 0, 0, 0};
+    // device copies
+    double *d_exp = nullptr, *d_ct = nullptr, *d_xyz = nullptr, *d_aofac = nullptr;
+    int *d_shell = nullptr, *d_off = nullptr, *d_by_l = nullptr, *d_shell_off = nullptr, *d_shell_pstart = nullptr;
+    const double* d_boys = nullptr;
+};
+
+struct te_pairs {
+    const te_basis* basis = nullptr;
+    double tau_pair = 0.0;
+    long long count[TE_NCLASS] = {0};
+    te::PairD* d_pair[TE_NCLASS] = {nullptr};
+    double* d_q[TE_NCLASS] = {nullptr};
+    te::PairIds* d_ids[TE_NCLASS] = {nullptr};
+    // per-build scratch
+    double *d_Ds = nullptr, *d_Jt = nullptr, *d_Kt = nullptr, *d_Dm = nullptr;
+    te::JKControl* d_ctrl = nullptr;
+    long long* d_tile_start = nullptr;
+    long long tile_cap = 0;
+    double *d_hD = nullptr, *d_hJ = nullptr, *d_hK = nullptr;   // staging for te_build_jk_host
+    bool profiling = false;
+    cudaStream_t last_stream = nullptr;
+    cudaEvent_t ev0[TE_NCLASS * TE_NCLASS] = {nullptr}, ev1[TE_NCLASS * TE_NCLASS] = {nullptr};
+};
+
+namespace te {
+// te_inst_*.cu
+int launch_schwarz(int la, int lb, const te_basis* b, long long ncand, double* d_q, long long* d_idx);
+int launch_pair_fill(int la, int lb, const te_basis* b, long long n, const long long* d_idx, PairD* d_pair, PairIds* d_ids);
+int launch_jk_class(int cb, int ck, te_pairs* P, double tau, cudaStream_t st);
+int launch_eri_class(int cb, int ck, const te_basis* b, int n, const EriTask* d_tasks, double* out_dev);
+}  // namespace te

@@ -1,0 +1,526 @@
+// te_lib.cu -- host side of the C ABI (include/te_jk.h): basis, pair builder, J/K build driver, Boys /
+// peak utilities.  Kernels for the per-class work live in te_kernels.cuh and are instantiated in te_inst_*.cu.
+#include "te_internal.h"
+
+#include <cub/cub.cuh>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <cstdlib>
+#include <new>
+#include <vector>
+
+namespace te {
+
+thread_local char g_err[512] = "";
+
+void set_error(const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+// ------------------------------------------------------------------------------------------ Boys table
+// F_m(T_i) for the Taylor grid of te_md.cuh, generated on the host in long double: convergent series at the
+// top m (all terms positive), then the downward recursion.
+static double* g_boys_tab = nullptr;   // device, [BOYS_NPTS][BOYS_MROWS]; one per process (single device)
+
+int ensure_boys_table(const double** out) {
+    if (!g_boys_tab) {
+        std::vector<double> h((size_t)BOYS_NPTS * BOYS_MROWS);
+        const int mtop = BOYS_MROWS - 1;
+        for (int i = 0; i < BOYS_NPTS; ++i) {
+            const long double T = (long double)i * (long double)BOYS_DT;
+            const long double eT = expl(-T);
+            long double term = 1.0L / (2 * mtop + 1), sum = term;
+            for (int k = 1; k < 2000; ++k) {
+                term *= 2.0L * T / (2 * mtop + 2 * k + 1);
+                sum += term;
+                if (term < 1e-22L * sum) break;
+            }
+            long double F = eT * sum;
+            h[(size_t)i * BOYS_MROWS + mtop] = (double)F;
+            for (int m = mtop; m > 0; --m) {
+                F = (2.0L * T * F + eT) / (2 * m - 1);
+                h[(size_t)i * BOYS_MROWS + m - 1] = (double)F;
+            }
+        }
+        double* d = nullptr;
+        TE_CUDA(cudaMalloc(&d, h.size() * sizeof(double)));
+        TE_CUDA(cudaMemcpy(d, h.data(), h.size() * sizeof(double), cudaMemcpyHostToDevice));
+        g_boys_tab = d;
+    }
+    *out = g_boys_tab;
+    return TE_OK;
+}
+
+template <class T>
+static int upload(const std::vector<T>& h, T** d) {
+    *d = nullptr;
+    if (h.empty()) return TE_OK;
+    TE_CUDA(cudaMalloc(d, h.size() * sizeof(T)));
+    TE_CUDA(cudaMemcpy(*d, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return TE_OK;
+}
+
+static double dfact(int n) { double r = 1.0; for (; n > 1; n -= 2) r *= n; return r; }
+
+}  // namespace te
+
+using namespace te;
+
+// ================================================================================================ basis
+extern "C" int te_basis_create(int natoms, const double* xyz, int nshells, const int* shell_atom, const int* shell_l,
+                               const int* shell_nprim, const double* exponents, const double* coefficients,
+                               te_basis** out) {
+    if (!out) { set_error("te_basis_create: out is NULL"); return TE_ERR_BAD_ARG; }
+    *out = nullptr;
+    if (natoms <= 0 || nshells <= 0 || !xyz || !shell_atom || !shell_l || !shell_nprim || !exponents || !coefficients) {
+        set_error("te_basis_create: empty basis or NULL argument");
+        return TE_ERR_BAD_ARG;
+    }
+    te_basis* b = new (std::nothrow) te_basis();
+    if (!b) { set_error("te_basis_create: out of host memory"); return TE_ERR_ALLOC; }
+    b->natoms = natoms; b->nshells = nshells;
+    int np = 0, nbf = 0;
+    for (int s = 0; s < nshells; ++s) {
+        if (shell_l[s] < 0 || shell_nprim[s] < 1 || shell_atom[s] < 0 || shell_atom[s] >= natoms) {
+            set_error("te_basis_create: shell %d has bad l / nprim / atom", s); delete b; return TE_ERR_BAD_ARG;
+        }
+        if (shell_l[s] > 3) { set_error("te_basis_create: shell %d has l = %d > 3", s, shell_l[s]); delete b; return TE_ERR_UNSUPPORTED_L; }
+        b->shell_l.push_back(shell_l[s]); b->shell_off.push_back(nbf); b->shell_pstart.push_back(np);
+        b->shell_nprim.push_back(shell_nprim[s]);
+        nbf += ncart(shell_l[s]); np += shell_nprim[s];
+    }
+    b->shell_off.push_back(nbf); b->shell_pstart.push_back(np);
+    b->nbf = nbf; b->nprim = np;
+    for (int i = 0; i < np; ++i)
+        if (!(exponents[i] > 0.0) || !std::isfinite(exponents[i]) || !std::isfinite(coefficients[i])) {
+            set_error("te_basis_create: primitive %d has a non-positive exponent or non-finite value", i); delete b; return TE_ERR_BAD_ARG;
+        }
+    // Normalisation (eq. 1-2): radial norm of the x^l primitive, N = (2a/pi)^{3/4} (4a)^{l/2} / sqrt((2l-1)!!);
+    // contracted self overlap of the x^l component S = sum c_m N_m c_n N_n (pi/p)^{3/2} (2l-1)!!/(2p)^l; c~ = cN/sqrt(S).
+    const double pi = 3.14159265358979323846;
+    std::vector<double> pxyz(3 * (size_t)np);
+    b->prim_exp.resize(np); b->prim_ct.resize(np); b->prim_l.resize(np); b->prim_shell.resize(np);
+    b->prim_iprim.resize(np); b->prim_off.resize(np);
+    for (int s = 0; s < nshells; ++s) {
+        const int l = shell_l[s], p0 = b->shell_pstart[s], n = shell_nprim[s];
+        std::vector<double> c(n);
+        for (int m = 0; m < n; ++m) {
+            const double a = exponents[p0 + m];
+            c[m] = coefficients[p0 + m] * std::pow(2.0 * a / pi, 0.75) * std::pow(4.0 * a, 0.5 * l) / std::sqrt(dfact(2 * l - 1));
+        }
+        double S = 0.0;
+        for (int m = 0; m < n; ++m)
+            for (int k = 0; k < n; ++k) {
+                const double p = exponents[p0 + m] + exponents[p0 + k];
+                S += c[m] * c[k] * std::pow(pi / p, 1.5) * dfact(2 * l - 1) / std::pow(2.0 * p, (double)l);
+            }
+        if (!(S > 0.0)) { set_error("te_basis_create: shell %d has zero norm", s); delete b; return TE_ERR_BAD_ARG; }
+        for (int m = 0; m < n; ++m) {
+            const int g = p0 + m;
+            b->prim_exp[g] = exponents[g]; b->prim_ct[g] = c[m] / std::sqrt(S); b->prim_l[g] = l;
+            b->prim_shell[g] = s; b->prim_iprim[g] = m; b->prim_off[g] = b->shell_off[s];
+            for (int d = 0; d < 3; ++d) pxyz[3 * (size_t)g + d] = xyz[3 * shell_atom[s] + d];
+        }
+    }
+    b->prim_xyz = pxyz;
+    // primitives grouped by l (the pair builder enumerates class candidates from these lists)
+    for (int l = 0; l < 4; ++l) {
+        b->l_start[l] = (int)b->prims_by_l.size();
+        for (int g = 0; g < np; ++g) if (b->prim_l[g] == l) b->prims_by_l.push_back(g);
+    }
+    b->l_start[4] = (int)b->prims_by_l.size();
+    std::vector<double> aofac(nbf);
+    for (int s = 0; s < nshells; ++s)
+        for (int i = 0; i < ncart(shell_l[s]); ++i) aofac[b->shell_off[s] + i] = comp_factor(shell_l[s], i);
+    int rc;
+    if ((rc = upload(b->prim_exp, &b->d_exp)) || (rc = upload(b->prim_ct, &b->d_ct)) || (rc = upload(b->prim_xyz, &b->d_xyz)) ||
+        (rc = upload(b->prim_shell, &b->d_shell)) || (rc = upload(b->prim_off, &b->d_off)) ||
+        (rc = upload(b->prims_by_l, &b->d_by_l)) || (rc = upload(aofac, &b->d_aofac)) ||
+        (rc = upload(b->shell_off, &b->d_shell_off)) || (rc = upload(b->shell_pstart, &b->d_shell_pstart)) || (rc = ensure_boys_table(&b->d_boys))) {
+        te_basis_destroy(b);
+        return rc;
+    }
+    *out = b;
+    return TE_OK;
+}
+
+extern "C" void te_basis_destroy(te_basis* b) {
+    if (!b) return;
+    cudaFree(b->d_exp); cudaFree(b->d_ct); cudaFree(b->d_xyz); cudaFree(b->d_shell); cudaFree(b->d_off);
+    cudaFree(b->d_by_l); cudaFree(b->d_aofac); cudaFree(b->d_shell_off); cudaFree(b->d_shell_pstart);
+    delete b;
+}
+
+extern "C" int te_basis_nbf(const te_basis* b) { return b ? b->nbf : TE_ERR_BAD_ARG; }
+extern "C" int te_basis_nprim(const te_basis* b) { return b ? b->nprim : TE_ERR_BAD_ARG; }
+
+extern "C" int te_basis_shell_offsets(const te_basis* b, int* offsets) {
+    if (!b || !offsets) { set_error("te_basis_shell_offsets: NULL argument"); return TE_ERR_BAD_ARG; }
+    std::memcpy(offsets, b->shell_off.data(), sizeof(int) * (b->nshells + 1));
+    return TE_OK;
+}
+
+extern "C" int te_basis_norm_coefs(const te_basis* b, double* norm) {
+    if (!b || !norm) { set_error("te_basis_norm_coefs: NULL argument"); return TE_ERR_BAD_ARG; }
+    std::memcpy(norm, b->prim_ct.data(), sizeof(double) * b->nprim);
+    return TE_OK;
+}
+
+// =========================================================================================== pair build
+__global__ void count_kept_kernel(const double* __restrict__ q_sorted, long long n, double tau, unsigned long long* out) {
+    // q_sorted is descending: count entries >= tau
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    unsigned long long c = 0;
+    for (; i < n; i += (long long)gridDim.x * blockDim.x) c += (q_sorted[i] >= tau) ? 1ull : 0ull;
+    for (int o = 16; o > 0; o >>= 1) c += __shfl_down_sync(0xffffffffu, c, o);
+    if ((threadIdx.x & 31) == 0 && c) atomicAdd(out, c);
+}
+
+extern "C" int te_shellpair_build(const te_basis* b, double tau_pair, te_pairs** out) {
+    if (!out) { set_error("te_shellpair_build: out is NULL"); return TE_ERR_BAD_ARG; }
+    *out = nullptr;
+    if (!b || !(tau_pair >= 0.0)) { set_error("te_shellpair_build: NULL basis or negative threshold"); return TE_ERR_BAD_ARG; }
+    te_pairs* P = new (std::nothrow) te_pairs();
+    if (!P) { set_error("te_shellpair_build: out of host memory"); return TE_ERR_ALLOC; }
+    P->basis = b; P->tau_pair = tau_pair;
+    unsigned long long* d_cnt = nullptr;
+    int rc = TE_OK;
+    auto fail = [&](int code) { cudaFree(d_cnt); te_pairs_destroy(P); return code; };
+    if (cudaMalloc(&d_cnt, sizeof(unsigned long long)) != cudaSuccess) { set_error("cudaMalloc failed"); return fail(TE_ERR_ALLOC); }
+    for (int la = 0; la < 4; ++la)
+        for (int lb = la; lb < 4; ++lb) {
+            const int cls = pair_class(la, lb);
+            const long long na = b->l_start[la + 1] - b->l_start[la], nb = b->l_start[lb + 1] - b->l_start[lb];
+            const long long ncand = (la == lb) ? na * (na + 1) / 2 : na * nb;
+            P->count[cls] = 0;
+            if (ncand == 0) continue;
+            double *d_q = nullptr, *d_qs = nullptr;
+            long long *d_idx = nullptr, *d_idxs = nullptr;
+            void* d_tmp = nullptr;
+            auto cleanup = [&]() { cudaFree(d_q); cudaFree(d_qs); cudaFree(d_idx); cudaFree(d_idxs); cudaFree(d_tmp); };
+            if (cudaMalloc(&d_q, ncand * sizeof(double)) != cudaSuccess || cudaMalloc(&d_qs, ncand * sizeof(double)) != cudaSuccess ||
+                cudaMalloc(&d_idx, ncand * sizeof(long long)) != cudaSuccess || cudaMalloc(&d_idxs, ncand * sizeof(long long)) != cudaSuccess) {
+                cleanup(); set_error("te_shellpair_build: device allocation of %lld candidates failed", ncand); return fail(TE_ERR_ALLOC);
+            }
+            // pass 1: Schwarz bound of every candidate (eq. 45), diagonal integral class (la lb|la lb)
+            if ((rc = launch_schwarz(la, lb, b, ncand, d_q, d_idx)) != TE_OK) { cleanup(); return fail(rc); }
+            // sort by bound, descending (radix sort: stable, so ties keep ascending candidate order)
+            size_t tmp_bytes = 0;
+            cub::DeviceRadixSort::SortPairsDescending(nullptr, tmp_bytes, d_q, d_qs, d_idx, d_idxs, (int)ncand);
+            if (cudaMalloc(&d_tmp, tmp_bytes) != cudaSuccess) { cleanup(); set_error("cub temp alloc failed"); return fail(TE_ERR_ALLOC); }
+            cub::DeviceRadixSort::SortPairsDescending(d_tmp, tmp_bytes, d_q, d_qs, d_idx, d_idxs, (int)ncand);
+            cudaMemset(d_cnt, 0, sizeof(unsigned long long));
+            count_kept_kernel<<<296, 256>>>(d_qs, ncand, tau_pair, d_cnt);
+            unsigned long long nk = 0;
+            if (cudaMemcpy(&nk, d_cnt, sizeof(nk), cudaMemcpyDeviceToHost) != cudaSuccess) {
+                cleanup(); set_error("te_shellpair_build: %s", cudaGetErrorString(cudaGetLastError())); return fail(TE_ERR_CUDA);
+            }
+            P->count[cls] = (long long)nk;
+            if (nk) {
+                // pass 2: pair data of the survivors in sorted order
+                if (cudaMalloc(&P->d_pair[cls], nk * sizeof(PairD)) != cudaSuccess || cudaMalloc(&P->d_q[cls], nk * sizeof(double)) != cudaSuccess ||
+                    cudaMalloc(&P->d_ids[cls], nk * sizeof(PairIds)) != cudaSuccess) {
+                    cleanup(); set_error("te_shellpair_build: pair allocation failed"); return fail(TE_ERR_ALLOC);
+                }
+                cudaMemcpy(P->d_q[cls], d_qs, nk * sizeof(double), cudaMemcpyDeviceToDevice);
+                if ((rc = launch_pair_fill(la, lb, b, (long long)nk, d_idxs, P->d_pair[cls], P->d_ids[cls])) != TE_OK) { cleanup(); return fail(rc); }
+            }
+            cudaError_t e = cudaDeviceSynchronize();
+            cleanup();
+            if (e != cudaSuccess) { set_error("te_shellpair_build: %s", cudaGetErrorString(e)); return fail(TE_ERR_CUDA); }
+        }
+    cudaFree(d_cnt);
+    // per-build scratch
+    const size_t n2 = (size_t)b->nbf * b->nbf, ns2 = (size_t)b->nshells * b->nshells;
+    if (cudaMalloc(&P->d_Ds, n2 * sizeof(double)) != cudaSuccess || cudaMalloc(&P->d_Jt, n2 * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&P->d_Kt, n2 * sizeof(double)) != cudaSuccess || cudaMalloc(&P->d_Dm, ns2 * sizeof(double)) != cudaSuccess ||
+        cudaMalloc(&P->d_ctrl, sizeof(JKControl)) != cudaSuccess) {
+        set_error("te_shellpair_build: scratch allocation failed"); te_pairs_destroy(P); return TE_ERR_ALLOC;
+    }
+    long long maxtiles = 0;
+    for (int c = 0; c < TE_NCLASS; ++c) maxtiles = std::max(maxtiles, P->count[c] / 4 + 2);
+    if (cudaMalloc(&P->d_tile_start, (maxtiles + 1) * sizeof(long long)) != cudaSuccess) {
+        set_error("te_shellpair_build: scratch allocation failed"); te_pairs_destroy(P); return TE_ERR_ALLOC;
+    }
+    P->tile_cap = maxtiles;
+    for (int i = 0; i < TE_NCLASS * TE_NCLASS; ++i) { cudaEventCreate(&P->ev0[i]); cudaEventCreate(&P->ev1[i]); }
+    *out = P;
+    return TE_OK;
+}
+
+extern "C" void te_pairs_destroy(te_pairs* P) {
+    if (!P) return;
+    for (int c = 0; c < TE_NCLASS; ++c) { cudaFree(P->d_pair[c]); cudaFree(P->d_q[c]); cudaFree(P->d_ids[c]); }
+    cudaFree(P->d_Ds); cudaFree(P->d_Jt); cudaFree(P->d_Kt); cudaFree(P->d_Dm); cudaFree(P->d_ctrl); cudaFree(P->d_tile_start);
+    cudaFree(P->d_hD); cudaFree(P->d_hJ); cudaFree(P->d_hK);
+    for (int i = 0; i < TE_NCLASS * TE_NCLASS; ++i) { if (P->ev0[i]) cudaEventDestroy(P->ev0[i]); if (P->ev1[i]) cudaEventDestroy(P->ev1[i]); }
+    delete P;
+}
+
+extern "C" int te_pairs_info(const te_pairs* P, long long class_count[TE_NCLASS], long long* nkept) {
+    if (!P) { set_error("te_pairs_info: NULL handle"); return TE_ERR_BAD_ARG; }
+    long long tot = 0;
+    for (int c = 0; c < TE_NCLASS; ++c) { if (class_count) class_count[c] = P->count[c]; tot += P->count[c]; }
+    if (nkept) *nkept = tot;
+    return TE_OK;
+}
+
+extern "C" int te_pairs_export(const te_pairs* P, int cls, int* shellA, int* shellB, int* primA, int* primB, double* bound) {
+    if (!P || cls < 0 || cls >= TE_NCLASS) { set_error("te_pairs_export: bad handle or class"); return TE_ERR_BAD_ARG; }
+    const long long n = P->count[cls];
+    if (n == 0) return TE_OK;
+    std::vector<PairIds> ids(n);
+    TE_CUDA(cudaMemcpy(ids.data(), P->d_ids[cls], n * sizeof(PairIds), cudaMemcpyDeviceToHost));
+    const te_basis* b = P->basis;
+    for (long long i = 0; i < n; ++i) {
+        if (shellA) shellA[i] = ids[i].shA;
+        if (shellB) shellB[i] = ids[i].shB;
+        if (primA) primA[i] = b->prim_iprim[ids[i].m];
+        if (primB) primB[i] = b->prim_iprim[ids[i].n];
+    }
+    if (bound) TE_CUDA(cudaMemcpy(bound, P->d_q[cls], n * sizeof(double), cudaMemcpyDeviceToHost));
+    return TE_OK;
+}
+
+extern "C" int te_pairs_export_geom(const te_pairs* P, int cls, double* P_xyz, double* p_exp, double* prefactor) {
+    if (!P || cls < 0 || cls >= TE_NCLASS) { set_error("te_pairs_export_geom: bad handle or class"); return TE_ERR_BAD_ARG; }
+    const long long n = P->count[cls];
+    if (n == 0) return TE_OK;
+    std::vector<PairD> pd(n);
+    TE_CUDA(cudaMemcpy(pd.data(), P->d_pair[cls], n * sizeof(PairD), cudaMemcpyDeviceToHost));
+    for (long long i = 0; i < n; ++i) {
+        if (P_xyz) for (int d = 0; d < 3; ++d) P_xyz[3 * i + d] = pd[i].P[d];
+        if (p_exp) p_exp[i] = pd[i].p;
+        if (prefactor) prefactor[i] = pd[i].pref;
+    }
+    return TE_OK;
+}
+
+// ============================================================================================= J/K build
+// Per-AO scaling by the component normalisation factor f (folded out of the integral kernels):
+// Ds = D o (f f^T) on input; J = (Jt + Jt^T) o (f f^T) on output (same for K).
+__global__ void scale_density_kernel(const double* __restrict__ D, const double* __restrict__ f, int nbf, double* __restrict__ Ds) {
+    const long long n2 = (long long)nbf * nbf;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < n2; x += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(x / nbf), j = (int)(x % nbf);
+        Ds[x] = D[x] * f[i] * f[j];
+    }
+}
+
+// Dm[X][Y] = max |D| over the block of contracted shells (X,Y); also the global maximum.
+__global__ void density_bounds_kernel(const double* __restrict__ D, const int* __restrict__ shell_off, int nshells, int nbf,
+                                      double* __restrict__ Dm, JKControl* ctrl) {
+    const long long ns2 = (long long)nshells * nshells;
+    double mx_all = 0.0;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < ns2; x += (long long)gridDim.x * blockDim.x) {
+        const int X = (int)(x / nshells), Y = (int)(x % nshells);
+        double mx = 0.0;
+        for (int i = shell_off[X]; i < shell_off[X + 1]; ++i)
+            for (int j = shell_off[Y]; j < shell_off[Y + 1]; ++j) mx = fmax(mx, fabs(D[(long long)i * nbf + j]));
+        Dm[x] = mx;
+        mx_all = fmax(mx_all, mx);
+    }
+    for (int o = 16; o > 0; o >>= 1) mx_all = fmax(mx_all, __shfl_down_sync(0xffffffffu, mx_all, o));
+    if ((threadIdx.x & 31) == 0) atomicMax(reinterpret_cast<unsigned long long*>(&ctrl->dmax), (unsigned long long)__double_as_longlong(mx_all));
+}
+
+__global__ void finish_kernel(const double* __restrict__ Jt, const double* __restrict__ Kt, const double* __restrict__ f, int nbf,
+                              double* __restrict__ J, double* __restrict__ K) {
+    const long long n2 = (long long)nbf * nbf;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < n2; x += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(x / nbf), j = (int)(x % nbf);
+        const long long y = (long long)j * nbf + i;
+        const double s = f[i] * f[j];
+        J[x] = (Jt[x] + Jt[y]) * s;
+        K[x] = (Kt[x] + Kt[y]) * s;
+    }
+}
+
+extern "C" int te_build_jk(const te_pairs* Pc, const double* D, double* J, double* K, double tau, void* stream_) {
+    te_pairs* P = const_cast<te_pairs*>(Pc);   // scratch and statistics live in the handle
+    if (!P || !D || !J || !K || !(tau >= 0.0)) { set_error("te_build_jk: NULL argument or negative threshold"); return TE_ERR_BAD_ARG; }
+    cudaStream_t st = (cudaStream_t)stream_;
+    const te_basis* b = P->basis;
+    const int nbf = b->nbf;
+    const size_t n2 = (size_t)nbf * nbf;
+    P->last_stream = st;
+    TE_CUDA(cudaMemsetAsync(P->d_Jt, 0, n2 * sizeof(double), st));
+    TE_CUDA(cudaMemsetAsync(P->d_Kt, 0, n2 * sizeof(double), st));
+    TE_CUDA(cudaMemsetAsync(P->d_ctrl, 0, sizeof(JKControl), st));
+    scale_density_kernel<<<592, 256, 0, st>>>(D, b->d_aofac, nbf, P->d_Ds);
+    density_bounds_kernel<<<592, 256, 0, st>>>(D, b->d_shell_off, b->nshells, nbf, P->d_Dm, P->d_ctrl);
+    int rc = TE_OK;
+    const char* only = getenv("TE_DEBUG_SLOT");   // debugging aid: run a single class pair "cb*10+ck"
+    for (int cb = 0; cb < TE_NCLASS && rc == TE_OK; ++cb)
+        for (int ck = cb; ck < TE_NCLASS && rc == TE_OK; ++ck) {
+            if (P->count[cb] == 0 || P->count[ck] == 0) continue;
+            if (only && atoi(only) != cb * TE_NCLASS + ck) continue;
+            const int slot = cb * TE_NCLASS + ck;
+            if (P->profiling) cudaEventRecord(P->ev0[slot], st);
+            rc = launch_jk_class(cb, ck, P, tau, st);
+            if (P->profiling) cudaEventRecord(P->ev1[slot], st);
+        }
+    if (rc != TE_OK) return rc;
+    finish_kernel<<<592, 256, 0, st>>>(P->d_Jt, P->d_Kt, b->d_aofac, nbf, J, K);
+    TE_CUDA(cudaGetLastError());
+    return TE_OK;
+}
+
+extern "C" int te_build_jk_host(const te_pairs* Pc, const double* D, double* J, double* K, double tau) {
+    te_pairs* P = const_cast<te_pairs*>(Pc);
+    if (!P || !D || !J || !K) { set_error("te_build_jk_host: NULL argument"); return TE_ERR_BAD_ARG; }
+    const size_t bytes = (size_t)P->basis->nbf * P->basis->nbf * sizeof(double);
+    if (!P->d_hD) {
+        if (cudaMalloc(&P->d_hD, bytes) != cudaSuccess || cudaMalloc(&P->d_hJ, bytes) != cudaSuccess || cudaMalloc(&P->d_hK, bytes) != cudaSuccess) {
+            set_error("te_build_jk_host: device allocation failed"); return TE_ERR_ALLOC;
+        }
+    }
+    TE_CUDA(cudaMemcpyAsync(P->d_hD, D, bytes, cudaMemcpyHostToDevice, 0));
+    int rc = te_build_jk(P, P->d_hD, P->d_hJ, P->d_hK, tau, nullptr);
+    if (rc != TE_OK) return rc;
+    TE_CUDA(cudaMemcpyAsync(J, P->d_hJ, bytes, cudaMemcpyDeviceToHost, 0));
+    TE_CUDA(cudaMemcpyAsync(K, P->d_hK, bytes, cudaMemcpyDeviceToHost, 0));
+    TE_CUDA(cudaStreamSynchronize(0));
+    return TE_OK;
+}
+
+extern "C" int te_jk_set_profiling(te_pairs* P, int on) {
+    if (!P) { set_error("te_jk_set_profiling: NULL handle"); return TE_ERR_BAD_ARG; }
+    P->profiling = on != 0;
+    return TE_OK;
+}
+
+extern "C" int te_jk_stats(const te_pairs* P, long long quartets[TE_NCLASS][TE_NCLASS], float ms[TE_NCLASS][TE_NCLASS]) {
+    if (!P) { set_error("te_jk_stats: NULL handle"); return TE_ERR_BAD_ARG; }
+    TE_CUDA(cudaStreamSynchronize(P->last_stream));
+    JKControl h;
+    TE_CUDA(cudaMemcpy(&h, P->d_ctrl, sizeof(h), cudaMemcpyDeviceToHost));
+    for (int cb = 0; cb < TE_NCLASS; ++cb)
+        for (int ck = 0; ck < TE_NCLASS; ++ck) {
+            const int slot = cb * TE_NCLASS + ck;
+            if (quartets) quartets[cb][ck] = (long long)h.live[slot];
+            if (ms) {
+                float t = 0.f;
+                if (P->profiling && ck >= cb && P->count[cb] && P->count[ck]) cudaEventElapsedTime(&t, P->ev0[slot], P->ev1[slot]);
+                ms[cb][ck] = t;
+            }
+        }
+    return TE_OK;
+}
+
+// ============================================================================================= utilities
+extern "C" int te_eri_block(const te_basis* b, int nq, const int* quartets, const long long* offs, double* out_dev) {
+    if (!b || nq < 0 || (nq > 0 && (!quartets || !offs || !out_dev))) { set_error("te_eri_block: NULL argument"); return TE_ERR_BAD_ARG; }
+    if (nq == 0) return TE_OK;
+    // canonicalise every quartet to la<=lb, lc<=ld, class(ab)<=class(cd); record output strides
+    std::vector<EriTask> tasks[TE_NCLASS * TE_NCLASS];
+    for (int x = 0; x < nq; ++x) {
+        int s[4], stride[4];
+        for (int k = 0; k < 4; ++k) {
+            s[k] = quartets[4 * x + k];
+            if (s[k] < 0 || s[k] >= b->nshells) { set_error("te_eri_block: quartet %d has shell id %d out of range", x, s[k]); return TE_ERR_BAD_ARG; }
+        }
+        const int n[4] = {ncart(b->shell_l[s[0]]), ncart(b->shell_l[s[1]]), ncart(b->shell_l[s[2]]), ncart(b->shell_l[s[3]])};
+        stride[0] = n[1] * n[2] * n[3]; stride[1] = n[2] * n[3]; stride[2] = n[3]; stride[3] = 1;
+        int o[4] = {0, 1, 2, 3};
+        if (b->shell_l[s[o[0]]] > b->shell_l[s[o[1]]]) std::swap(o[0], o[1]);
+        if (b->shell_l[s[o[2]]] > b->shell_l[s[o[3]]]) std::swap(o[2], o[3]);
+        int cb = pair_class(b->shell_l[s[o[0]]], b->shell_l[s[o[1]]]), ck = pair_class(b->shell_l[s[o[2]]], b->shell_l[s[o[3]]]);
+        if (cb > ck) { std::swap(o[0], o[2]); std::swap(o[1], o[3]); std::swap(cb, ck); }
+        EriTask t;
+        for (int k = 0; k < 4; ++k) { t.sh[k] = s[o[k]]; t.stride[k] = stride[o[k]]; }
+        t.out = offs[x];
+        if (offs[x + 1] - offs[x] != (long long)n[0] * n[1] * n[2] * n[3]) { set_error("te_eri_block: out_offsets of quartet %d do not match its size", x); return TE_ERR_BAD_ARG; }
+        tasks[cb * TE_NCLASS + ck].push_back(t);
+    }
+    TE_CUDA(cudaMemset(out_dev, 0, (size_t)offs[nq] * sizeof(double)));
+    for (int cb = 0; cb < TE_NCLASS; ++cb)
+        for (int ck = cb; ck < TE_NCLASS; ++ck) {
+            auto& v = tasks[cb * TE_NCLASS + ck];
+            if (v.empty()) continue;
+            EriTask* d = nullptr;
+            int rc = upload(v, &d);
+            if (rc == TE_OK) rc = launch_eri_class(cb, ck, b, (int)v.size(), d, out_dev);
+            cudaError_t e = cudaDeviceSynchronize();
+            cudaFree(d);
+            if (rc != TE_OK) return rc;
+            if (e != cudaSuccess) { set_error("te_eri_block: %s", cudaGetErrorString(e)); return TE_ERR_CUDA; }
+        }
+    return TE_OK;
+}
+
+template <int L>
+__global__ void boys_kernel(int n, const double* __restrict__ T, const double* __restrict__ tab, double* __restrict__ F) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double f[L + 1];
+    boys<L>(T[i], tab, f);
+#pragma unroll
+    for (int m = 0; m <= L; ++m) F[(size_t)i * (L + 1) + m] = f[m];
+}
+
+template <int L>
+static void boys_dispatch(int mmax, int n, const double* T, const double* tab, double* F) {
+    if (mmax == L) boys_kernel<L><<<(n + 127) / 128, 128>>>(n, T, tab, F);
+    else if constexpr (L > 0) boys_dispatch<L - 1>(mmax, n, T, tab, F);
+}
+
+extern "C" int te_boys(int n, const double* T_dev, int mmax, double* F_dev) {
+    if (n < 0 || mmax < 0 || mmax > 12 || (n > 0 && (!T_dev || !F_dev))) { set_error("te_boys: bad argument"); return TE_ERR_BAD_ARG; }
+    if (n == 0) return TE_OK;
+    const double* tab;
+    int rc = ensure_boys_table(&tab);
+    if (rc) return rc;
+    boys_dispatch<12>(mmax, n, T_dev, tab, F_dev);
+    TE_CUDA(cudaDeviceSynchronize());
+    return TE_OK;
+}
+
+// Register-resident DFMA chains: 8 independent accumulators per thread, every SM busy.
+__global__ void __launch_bounds__(256) dfma_peak_kernel(double* out, int iters, double a, double b) {
+    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+            x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+        }
+    }
+    out[blockIdx.x * blockDim.x + threadIdx.x] = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
+}
+
+extern "C" int te_measure_fp64_peak(double* tflops) {
+    if (!tflops) { set_error("te_measure_fp64_peak: NULL argument"); return TE_ERR_BAD_ARG; }
+    int dev = 0, sms = 0;
+    TE_CUDA(cudaGetDevice(&dev));
+    TE_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int blocks = sms * 8, threads = 256, iters = 4096;
+    double* d = nullptr;
+    TE_CUDA(cudaMalloc(&d, (size_t)blocks * threads * sizeof(double)));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {
+        cudaEventRecord(e0);
+        dfma_peak_kernel<<<blocks, threads>>>(d, iters, 0.999999, 1e-9);
+        cudaEventRecord(e1);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double fl = 2.0 * 8 * 16 * (double)iters * blocks * threads;
+        if (rep > 0) best = std::max(best, fl / (ms * 1e-3) / 1e12);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+    TE_CUDA(cudaGetLastError());
+    *tflops = best;
+    return TE_OK;
+}
+
+extern "C" const char* te_last_error(void) { return te::g_err; }
