@@ -1,6 +1,8 @@
 // te_inst.cu -- instantiates every kernel whose BRA pair class is TE_CB (compiled 10 times, -DTE_CB=0..9, so the
 // 55 (la lb|lc ld) classes build in parallel).  Exposes launch_*_cb<TE_CB> entry points used by te_dispatch.cu.
-#include "te_kernels.cuh"
+#include "te_jkw.cuh"
+
+#include <cstdlib>
 
 #ifndef TE_CB
 #error "compile with -DTE_CB=<bra class 0..9>"
@@ -45,14 +47,33 @@ static int jk_launch(te_pairs* P, double tau, cudaStream_t st) {
     a.Ds = P->d_Ds; a.Dm = P->d_Dm; a.Jt = P->d_Jt; a.Kt = P->d_Kt; a.boys_tab = b->d_boys;
     a.tile_start = P->d_tile_start; a.ctrl = P->d_ctrl; a.tau = tau; a.nbf = b->nbf; a.nshells = b->nshells;
     a.slot = slot; a.same = (TE_CB == CK);
-    schedule_kernel<<<1, 1024, 0, st>>>(a.qb, a.nb, a.qk, a.nk, a.same, tau, TB, TK, P->d_tile_start, P->d_ctrl, slot);
+    a.task_hi = P->d_task_hi;
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const long long max_tiles = ((a.nb + TB - 1) / TB) * ((a.nk + TK - 1) / TK);
-    const int per_sm = light ? 8 : 16;   // resident CTAs per SM worth of persistent blocks
-    const unsigned grid = (unsigned)std::min<long long>(max_tiles, (long long)sms * per_sm);
-    jk_kernel<LA, LB, LC, LD, TB, TK><<<grid, TB * TK, 0, st>>>(a);
+    static const int impl = getenv("TE_JK_IMPL") ? atoi(getenv("TE_JK_IMPL")) : 1;   // 0: generic thread-per-quartet kernel everywhere
+    if (light || impl == 0) {
+        schedule_kernel<<<1, 1024, 0, st>>>(a.qb, a.nb, a.qk, a.nk, a.same, tau, TB, TK, P->d_tile_start, P->d_ctrl, slot);
+        const long long max_tiles = ((a.nb + TB - 1) / TB) * ((a.nk + TK - 1) / TK);
+        const int per_sm = light ? 8 : 16;   // resident CTAs per SM worth of persistent blocks
+        const unsigned grid = (unsigned)std::min<long long>(max_tiles, (long long)sms * per_sm);
+        jk_kernel<LA, LB, LC, LD, TB, TK><<<grid, TB * TK, 0, st>>>(a);
+    } else {
+        // uniform-ket kernel: one warp per block, per-lane R tensor in shared memory
+        using S = WShape<LA, LB, LC, LD>;
+        constexpr int smem = S::smem_doubles * (int)sizeof(double);
+        static int blocks_per_sm = 0;
+        if (!blocks_per_sm) {
+            TE_CUDA(cudaFuncSetAttribute(jkw_kernel<LA, LB, LC, LD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            TE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, jkw_kernel<LA, LB, LC, LD>, WARP, smem));
+            if (blocks_per_sm < 1) { set_error("jkw_kernel<%d,%d,%d,%d>: %d bytes of shared memory do not fit", LA, LB, LC, LD, smem); blocks_per_sm = 0; return TE_ERR_CUDA; }
+        }
+        const int warps = sms * blocks_per_sm;
+        schedule_w_kernel<<<1, 1024, 0, st>>>(a.qb, a.nb, a.qk, a.nk, a.same, tau, warps, P->d_tile_start, P->d_task_hi, P->d_ctrl, slot);
+        const long long max_tasks = a.nk * ((a.nb + WARP - 1) / WARP);
+        const unsigned grid = (unsigned)std::min<long long>(max_tasks, (long long)warps);
+        jkw_kernel<LA, LB, LC, LD><<<grid, WARP, smem, st>>>(a);
+    }
     TE_CUDA(cudaGetLastError());
     return TE_OK;
 }

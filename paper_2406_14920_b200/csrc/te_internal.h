@@ -31,6 +31,7 @@ struct JKControl {
     unsigned long long live[TE_NCLASS * TE_NCLASS];     // unique live quartets per class pair
     unsigned long long ntiles[TE_NCLASS * TE_NCLASS];   // scheduled tiles per class pair
     unsigned int tile_counter[TE_NCLASS * TE_NCLASS];   // dynamic tile queue heads
+    int chunk[TE_NCLASS * TE_NCLASS];                   // uniform-ket kernel: bras per task = 32 * chunk
 };
 
 struct EriTask {
@@ -64,11 +65,13 @@ struct te_pairs {
     double *d_Ds = nullptr, *d_Jt = nullptr, *d_Kt = nullptr, *d_Dm = nullptr;
     te::JKControl* d_ctrl = nullptr;
     long long* d_tile_start = nullptr;
+    int* d_task_hi = nullptr;
     long long tile_cap = 0;
     double *d_hD = nullptr, *d_hJ = nullptr, *d_hK = nullptr;   // staging for te_build_jk_host
     bool profiling = false;
     cudaStream_t last_stream = nullptr;
     cudaEvent_t ev0[TE_NCLASS * TE_NCLASS] = {nullptr}, ev1[TE_NCLASS * TE_NCLASS] = {nullptr};
+    bool ev_valid[TE_NCLASS * TE_NCLASS] = {false};
 };
 
 namespace te {

@@ -1,0 +1,413 @@
+// te_jkw.cuh -- "uniform-ket" J/K kernel: one warp = one KET primitive pair (warp-uniform) x 32 BRA primitive pairs (one per
+// lane).  Everything that depends only on the ket -- its Hermite expansion coefficients E_Q^{kl} (eq. 5-8), folded with the
+// (-1)^{t'+u'+v'} of eq. 30 and the pair prefactor, and its density block -- is built once per task in shared memory and read by
+// broadcast; every lane keeps its own R^0_{tuv} tensor (eq. 21-25) in a conflict-free shared-memory column and its bra
+// quantities in registers.  Per ket component pair (k,l) the lane forms
+//     Y_P  = sum_{Q in box(kl)} E~_Q^{kl} R_{P+Q}            (ket Hermite -> Cartesian, eq. 31 inner bracket)
+//     I_ij = pref * sum_P E_P^{ij} Y_P                       (bra Hermite -> Cartesian)
+// and digests I_ij into the two J and four K updates of the quartet (eq. 34, 36) with the per-term masks of eq. 47.
+#pragma once
+#include "te_kernels.cuh"
+
+namespace te {
+
+// ROW[L][t][u] = index of (t,u,0) in the nested tetrahedral layout tidx<L>; (t,u,v) sits v entries further.
+struct RowTab {
+    unsigned short v[13 * 13 * 13];
+    constexpr RowTab() : v{} {
+        for (int L = 0; L < 13; ++L)
+            for (int t = 0; t < 13; ++t)
+                for (int u = 0; u < 13; ++u) {
+                    const int a = L - t;
+                    v[(L * 13 + t) * 13 + u] = (t <= L && u <= a)
+                        ? (unsigned short)(((L + 1) * (L + 2) * (L + 3) - (a + 1) * (a + 2) * (a + 3)) / 6 + u * (a + 1) - u * (u - 1) / 2)
+                        : (unsigned short)0;
+                }
+    }
+};
+static __constant__ RowTab c_rowtab = RowTab();
+
+constexpr int WARP = 32;
+
+template <int LA, int LB, int LC, int LD>
+struct WShape {
+    static constexpr int LAB = LA + LB, LCD = LC + LD, L = LAB + LCD;
+    static constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
+    static constexpr int NHB = nherm(LAB), NR = nherm(L);
+    static constexpr int NNZK = nnz_e(LC, LD);
+    static constexpr int NE1 = (LC + 1) * (LD + 1) * (LCD + 1);
+    // K_?c accumulators / D_?c blocks of the smaller ket shell stay in registers for the whole quartet when small
+    static constexpr bool KEEPC = (NA + NB) * NC <= 24;
+    static constexpr int smem_doubles = NR * WARP + NNZK + 3 * NE1 + NC * ND;
+};
+
+// R^0_{tuv} of eq. 21-25 built in place in a shared-memory column (element i at R[i * 32]); same sweep as rtable<L>.
+template <int L>
+__device__ __forceinline__ void rtable_sm(double alpha, double X, double Y, double Z, const double* __restrict__ F, double* R) {
+    double fac[L + 1];
+    fac[0] = 1.0;
+#pragma unroll
+    for (int m = 1; m <= L; ++m) fac[m] = fac[m - 1] * (-2.0 * alpha);
+    R[0] = fac[L] * F[L];
+#pragma unroll
+    for (int m = L - 1; m >= 0; --m) {
+#pragma unroll
+        for (int n = L - m; n >= 1; --n) {
+#pragma unroll
+            for (int t = n; t >= 0; --t) {
+#pragma unroll
+                for (int u = n - t; u >= 0; --u) {
+                    const int v = n - t - u;
+                    double r;
+                    if (t > 0) {
+                        r = X * R[tidx<L>(t - 1, u, v) * WARP];
+                        if (t > 1) r = fma((double)(t - 1), R[tidx<L>(t - 2, u, v) * WARP], r);
+                    } else if (u > 0) {
+                        r = Y * R[tidx<L>(t, u - 1, v) * WARP];
+                        if (u > 1) r = fma((double)(u - 1), R[tidx<L>(t, u - 2, v) * WARP], r);
+                    } else {
+                        r = Z * R[tidx<L>(t, u, v - 1) * WARP];
+                        if (v > 1) r = fma((double)(v - 1), R[tidx<L>(t, u, v - 2) * WARP], r);
+                    }
+                    R[tidx<L>(t, u, v) * WARP] = r;
+                }
+            }
+        }
+        R[0] = fac[m] * F[m];
+    }
+}
+
+template <int LA, int LB, int LC, int LD>
+__global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
+    using S = WShape<LA, LB, LC, LD>;
+    constexpr int LAB = S::LAB, LCD = S::LCD, L = S::L;
+    constexpr int NA = S::NA, NB = S::NB, NC = S::NC, ND = S::ND, NHB = S::NHB;
+    constexpr bool KEEPC = S::KEEPC;
+    constexpr unsigned FULLMASK = 0xffffffffu;
+    extern __shared__ double sm[];
+    double* const Rsm = sm;
+    double* const kt = Rsm + S::NR * WARP;
+    double* const e1 = kt + S::NNZK;
+    double* const dcd = e1 + 3 * S::NE1;
+    const int lane = threadIdx.x;
+    double* const Rl = Rsm + lane;
+    const unsigned short* const rowtab = c_rowtab.v + L * 169;
+
+    const unsigned long long ntasks = a.ctrl->ntiles[a.slot];
+    const long long span = (long long)WARP * a.ctrl->chunk[a.slot];
+    const long long ns = a.nshells;
+    const long long nbf = a.nbf;
+    long long cached_j = -1;
+    PairD kp;
+    PairIds ik;
+    double qk = 0.0;
+    unsigned int nlive = 0;
+
+    while (true) {
+        unsigned int task = 0;
+        if (lane == 0) task = atomicAdd(&a.ctrl->tile_counter[a.slot], 1u);
+        task = __shfl_sync(FULLMASK, task, 0);
+        if (task >= ntasks) break;
+        long long lo = 0, hi = a.nk;   // last ket j with tile_start[j] <= task
+        while (hi - lo > 1) { const long long mid = (lo + hi) >> 1; if ((unsigned long long)a.tile_start[mid] <= task) lo = mid; else hi = mid; }
+        const long long j = lo;
+        const long long b_lo = (a.same ? j : 0) + ((long long)task - a.tile_start[j]) * span;
+        const long long b_hi = min((long long)a.task_hi[j], b_lo + span);
+
+        if (j != cached_j) {
+            // ---- ket-uniform tables: 1-D E coefficients (signed), their products per (k,l,Q) in loop order, density block
+            __syncwarp();
+            kp = a.pk[j]; ik = a.ik[j]; qk = a.qk[j];
+            if (lane < 3) {
+                double E[LC + 1][LD + 1][LCD + 1];
+                const double PA = lane == 0 ? kp.PA[0] : (lane == 1 ? kp.PA[1] : kp.PA[2]);
+                const double PB = lane == 0 ? kp.PB[0] : (lane == 1 ? kp.PB[1] : kp.PB[2]);
+                etable<LC, LD, true>(PA, PB, 0.5 / kp.p, E);
+#pragma unroll
+                for (int i = 0; i <= LC; ++i)
+#pragma unroll
+                    for (int jj = 0; jj <= LD; ++jj)
+#pragma unroll
+                        for (int t = 0; t <= LCD; ++t) e1[lane * S::NE1 + (i * (LD + 1) + jj) * (LCD + 1) + t] = E[i][jj][t];
+            }
+            __syncwarp();
+            int e = 0;
+            for (int l = 0; l < ND; ++l) {
+                const int lx = cart_x(LD, l), ly = cart_y(LD, l), lz = cart_z(LD, l);
+                for (int k = 0; k < NC; ++k) {
+                    const int kx = cart_x(LC, k), ky = cart_y(LC, k), kz = cart_z(LC, k);
+                    const double* ex = e1 + (kx * (LD + 1) + lx) * (LCD + 1);
+                    const double* ey = e1 + S::NE1 + (ky * (LD + 1) + ly) * (LCD + 1);
+                    const double* ez = e1 + 2 * S::NE1 + (kz * (LD + 1) + lz) * (LCD + 1);
+                    for (int t2 = 0; t2 <= kx + lx; ++t2)
+                        for (int u2 = 0; u2 <= ky + ly; ++u2)
+                            for (int v2 = 0; v2 <= kz + lz; ++v2, ++e)
+                                if ((e & 31) == lane) kt[e] = ex[t2] * ey[u2] * ez[v2] * kp.pref;
+                }
+            }
+            for (int cd = lane; cd < NC * ND; cd += WARP) dcd[cd] = a.Ds[(ik.offA + cd / ND) * nbf + ik.offB + cd % ND];
+            __syncwarp();
+            cached_j = j;
+        }
+
+        for (long long b0 = b_lo; b0 < b_hi; b0 += WARP) {
+            const long long bi = b0 + lane;
+            bool active = bi < b_hi;
+            PairD bp;
+            PairIds ib;
+            bool live_jab = false, live_jcd = false, live_kac = false, live_kbc = false, live_kad = false, live_kbd = false;
+            if (active) {
+                ib = a.ib[bi];
+                const double qq = a.qb[bi] * qk;
+                live_jab = qq * a.Dm[ik.shA * ns + ik.shB] >= a.tau;
+                live_jcd = qq * a.Dm[ib.shA * ns + ib.shB] >= a.tau;
+                live_kac = qq * a.Dm[ib.shB * ns + ik.shB] >= a.tau;
+                live_kbc = qq * a.Dm[ib.shA * ns + ik.shB] >= a.tau;
+                live_kad = qq * a.Dm[ib.shB * ns + ik.shA] >= a.tau;
+                live_kbd = qq * a.Dm[ib.shA * ns + ik.shA] >= a.tau;
+                active = live_jab | live_jcd | live_kac | live_kbc | live_kad | live_kbd;
+            }
+            if (!__any_sync(FULLMASK, active)) continue;
+            const bool any_jcd = __any_sync(FULLMASK, live_jcd);
+            double f = 1.0;
+            double Ebx[LA + 1][LB + 1][LAB + 1], Eby[LA + 1][LB + 1][LAB + 1], Ebz[LA + 1][LB + 1][LAB + 1];
+            double dab[NA * NB], jab[NA * NB];
+            double dbc[KEEPC ? NB * NC : 1], dac[KEEPC ? NA * NC : 1], kac[KEEPC ? NA * NC : 1], kbc[KEEPC ? NB * NC : 1];
+            const double* Da = nullptr; const double* Db = nullptr;   // rows of the scaled density at the bra's AOs
+            if (active) {
+                ++nlive;
+                bp = a.pb[bi];
+                if (ib.m == ib.n) f *= 0.5;
+                if (ik.m == ik.n) f *= 0.5;
+                if (a.same && bi == j) f *= 0.5;
+                const double p = bp.p, q = kp.p, pq = p + q;
+                const double alpha = p * q / pq;
+                const double X = bp.P[0] - kp.P[0], Y = bp.P[1] - kp.P[1], Z = bp.P[2] - kp.P[2];
+                double F[L + 1];
+                boys<L>(alpha * (X * X + Y * Y + Z * Z), a.boys_tab, F);
+                // 2 pi^{5/2} / (p q sqrt(p+q)) (eq. 30) x bra prefactor x symmetry factor, folded into the Boys values
+                const double pref = 34.986836655249725693 / (p * q * sqrt(pq)) * bp.pref * f;
+#pragma unroll
+                for (int m = 0; m <= L; ++m) F[m] *= pref;
+                rtable_sm<L>(alpha, X, Y, Z, F, Rl);
+                const double hb = 0.5 / p;
+                etable<LA, LB, false>(bp.PA[0], bp.PB[0], hb, Ebx);
+                etable<LA, LB, false>(bp.PA[1], bp.PB[1], hb, Eby);
+                etable<LA, LB, false>(bp.PA[2], bp.PB[2], hb, Ebz);
+                Da = a.Ds + (long long)ib.offA * nbf;
+                Db = a.Ds + (long long)ib.offB * nbf;
+#pragma unroll
+                for (int i = 0; i < NA; ++i)
+#pragma unroll
+                    for (int jj = 0; jj < NB; ++jj) { dab[i * NB + jj] = Da[i * nbf + ib.offB + jj]; jab[i * NB + jj] = 0.0; }
+                if (KEEPC) {
+#pragma unroll
+                    for (int k = 0; k < NC; ++k) {
+#pragma unroll
+                        for (int i = 0; i < NA; ++i) { dac[i * NC + k] = Da[i * nbf + ik.offA + k]; kac[i * NC + k] = 0.0; }
+#pragma unroll
+                        for (int jj = 0; jj < NB; ++jj) { dbc[jj * NC + k] = Db[jj * nbf + ik.offA + k]; kbc[jj * NC + k] = 0.0; }
+                    }
+                }
+            }
+            int ptr = 0;
+            for (int l = 0; l < ND; ++l) {
+                const int lx = cart_x(LD, l), ly = cart_y(LD, l), lz = cart_z(LD, l);
+                double dal[NA], dbl[NB], kal[NA], kbl[NB];
+                if (active) {
+#pragma unroll
+                    for (int i = 0; i < NA; ++i) { dal[i] = Da[i * nbf + ik.offB + l]; kal[i] = 0.0; }
+#pragma unroll
+                    for (int jj = 0; jj < NB; ++jj) { dbl[jj] = Db[jj * nbf + ik.offB + l]; kbl[jj] = 0.0; }
+                }
+                for (int k = 0; k < NC; ++k) {
+                    const int sx = cart_x(LC, k) + lx, sy = cart_y(LC, k) + ly, sz = cart_z(LC, k) + lz;
+                    double jkl = 0.0;
+                    if (active) {
+                        // ---- ket Hermite -> Cartesian for this (k,l): Y_P = sum_Q E~_Q R_{P+Q}
+                        double Yv[NHB];
+#pragma unroll
+                        for (int P = 0; P < NHB; ++P) Yv[P] = 0.0;
+                        const double* ktp = kt + ptr;
+                        for (int t2 = 0; t2 <= sx; ++t2)
+                            for (int u2 = 0; u2 <= sy; ++u2) {
+                                const unsigned short* rt = rowtab + t2 * 13 + u2;
+                                for (int v2 = 0; v2 <= sz; ++v2) {
+                                    const double e = *ktp++;
+                                    const double* Rq = Rl + v2 * WARP;
+#pragma unroll
+                                    for (int t = 0; t <= LAB; ++t)
+#pragma unroll
+                                        for (int u = 0; u <= LAB - t; ++u) {
+                                            const double* Rrow = Rq + (int)rt[t * 13 + u] * WARP;
+#pragma unroll
+                                            for (int v = 0; v <= LAB - t - u; ++v)
+                                                Yv[tidx<LAB>(t, u, v)] = fma(e, Rrow[v * WARP], Yv[tidx<LAB>(t, u, v)]);
+                                        }
+                                }
+                            }
+                        // ---- bra Hermite -> Cartesian and digestion
+                        double dbk[KEEPC ? 1 : NB], dak[KEEPC ? 1 : NA], kak[KEEPC ? 1 : NA], kbk[KEEPC ? 1 : NB];
+                        if (!KEEPC) {
+#pragma unroll
+                            for (int i = 0; i < NA; ++i) { dak[i] = Da[i * nbf + ik.offA + k]; kak[i] = 0.0; }
+#pragma unroll
+                            for (int jj = 0; jj < NB; ++jj) { dbk[jj] = Db[jj * nbf + ik.offA + k]; kbk[jj] = 0.0; }
+                        }
+                        const double dkl = dcd[k * ND + l];
+#pragma unroll
+                        for (int i = 0; i < NA; ++i) {
+                            const int ix = cart_x(LA, i), iy = cart_y(LA, i), iz = cart_z(LA, i);
+#pragma unroll
+                            for (int jj = 0; jj < NB; ++jj) {
+                                const int jx = cart_x(LB, jj), jy = cart_y(LB, jj), jz = cart_z(LB, jj);
+                                double s = 0.0;
+#pragma unroll
+                                for (int t = 0; t <= ix + jx; ++t) {
+                                    double su = 0.0;
+#pragma unroll
+                                    for (int u = 0; u <= iy + jy; ++u) {
+                                        double sv = 0.0;
+#pragma unroll
+                                        for (int v = 0; v <= iz + jz; ++v) sv = fma(Ebz[iz][jz][v], Yv[tidx<LAB>(t, u, v)], sv);
+                                        su = fma(Eby[iy][jy][u], sv, su);
+                                    }
+                                    s = fma(Ebx[ix][jx][t], su, s);
+                                }
+                                // s = f (ij|kl) without the per-component factors
+                                jab[i * NB + jj] = fma(s, dkl, jab[i * NB + jj]);
+                                jkl = fma(s, dab[i * NB + jj], jkl);
+                                if (KEEPC) {
+                                    kac[i * NC + k] = fma(s, dbl[jj], kac[i * NC + k]);
+                                    kbc[jj * NC + k] = fma(s, dal[i], kbc[jj * NC + k]);
+                                    kal[i] = fma(s, dbc[jj * NC + k], kal[i]);
+                                    kbl[jj] = fma(s, dac[i * NC + k], kbl[jj]);
+                                } else {
+                                    kak[i] = fma(s, dbl[jj], kak[i]);
+                                    kbk[jj] = fma(s, dal[i], kbk[jj]);
+                                    kal[i] = fma(s, dbk[jj], kal[i]);
+                                    kbl[jj] = fma(s, dak[i], kbl[jj]);
+                                }
+                            }
+                        }
+                        if (!KEEPC) {
+                            if (live_kac) {
+#pragma unroll
+                                for (int i = 0; i < NA; ++i) atomicAdd(&a.Kt[(ib.offA + i) * nbf + ik.offA + k], kak[i]);
+                            }
+                            if (live_kbc) {
+#pragma unroll
+                                for (int jj = 0; jj < NB; ++jj) atomicAdd(&a.Kt[(ib.offB + jj) * nbf + ik.offA + k], kbk[jj]);
+                            }
+                        }
+                        if (!live_jcd) jkl = 0.0;
+                    }
+                    ptr += (sx + 1) * (sy + 1) * (sz + 1);
+                    if (any_jcd) {
+#pragma unroll
+                        for (int o = 16; o > 0; o >>= 1) jkl += __shfl_xor_sync(FULLMASK, jkl, o);
+                        if (lane == 0) atomicAdd(&a.Jt[(ik.offA + k) * nbf + ik.offB + l], 2.0 * jkl);
+                    }
+                }
+                if (active) {
+                    if (live_kad) {
+#pragma unroll
+                        for (int i = 0; i < NA; ++i) atomicAdd(&a.Kt[(ib.offA + i) * nbf + ik.offB + l], kal[i]);
+                    }
+                    if (live_kbd) {
+#pragma unroll
+                        for (int jj = 0; jj < NB; ++jj) atomicAdd(&a.Kt[(ib.offB + jj) * nbf + ik.offB + l], kbl[jj]);
+                    }
+                }
+            }
+            if (active) {
+                if (live_jab) {
+#pragma unroll
+                    for (int i = 0; i < NA; ++i)
+#pragma unroll
+                        for (int jj = 0; jj < NB; ++jj) atomicAdd(&a.Jt[(ib.offA + i) * nbf + ib.offB + jj], 2.0 * jab[i * NB + jj]);
+                }
+                if (KEEPC) {
+                    if (live_kac) {
+#pragma unroll
+                        for (int i = 0; i < NA; ++i)
+#pragma unroll
+                            for (int k = 0; k < NC; ++k) atomicAdd(&a.Kt[(ib.offA + i) * nbf + ik.offA + k], kac[i * NC + k]);
+                    }
+                    if (live_kbc) {
+#pragma unroll
+                        for (int jj = 0; jj < NB; ++jj)
+#pragma unroll
+                            for (int k = 0; k < NC; ++k) atomicAdd(&a.Kt[(ib.offB + jj) * nbf + ik.offA + k], kbc[jj * NC + k]);
+                    }
+                }
+            }
+            __syncwarp();
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) nlive += __shfl_down_sync(FULLMASK, nlive, o);
+    if (lane == 0 && nlive) atomicAdd(&a.ctrl->live[a.slot], (unsigned long long)nlive);
+}
+
+// Task schedule of the uniform-ket kernel.  For ket j the live bras are a contiguous range of the (bound-sorted) bra list:
+// [same ? j : 0, cut_j) with cut_j = first bra whose q_bra * q_ket[j] * max|D| < tau (eq. 47, loosest density bound); a task is
+// (ket j, chunk of 32*chunk bras).  task_hi[j] = cut_j, tile_start = exclusive prefix sum of the chunk counts.
+static __global__ void __launch_bounds__(1024) schedule_w_kernel(const double* __restrict__ qb, long long nb, const double* __restrict__ qk,
+                                                          long long nk, int same, double tau, int target_warps,
+                                                          long long* __restrict__ tile_start, int* __restrict__ task_hi, JKControl* ctrl, int slot) {
+    __shared__ long long part[1024];
+    __shared__ int s_chunk;
+    const long long per = (nk + blockDim.x - 1) / blockDim.x;
+    const long long j0 = threadIdx.x * per, j1 = min(nk, j0 + per);
+    const double dmax = ctrl->dmax;
+    long long tot = 0;
+    for (long long j = j0; j < j1; ++j) {
+        long long cut;
+        if (tau <= 0.0) cut = nb;
+        else {
+            const double w = qk[j] * dmax;
+            if (!(w > 0.0)) cut = 0;
+            else {
+                const double thr = tau / w * (1.0 - 1e-12);
+                long long lo = 0, hi = nb;   // first bra index with qb < thr
+                while (lo < hi) { const long long mid = (lo + hi) >> 1; if (qb[mid] >= thr) lo = mid + 1; else hi = mid; }
+                cut = lo;
+            }
+        }
+        const long long lo_j = same ? j : 0;
+        if (cut < lo_j) cut = lo_j;
+        task_hi[j] = (int)cut;
+        tot += cut - lo_j;
+    }
+    part[threadIdx.x] = tot;
+    __syncthreads();
+    for (int o = blockDim.x >> 1; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) part[threadIdx.x] += part[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        // chunk: 32*chunk bras per task, sized so every resident warp gets ~8 tasks; 1..16
+        long long c = part[0] / ((long long)WARP * target_warps * 8);
+        s_chunk = (int)max(1LL, min(16LL, c));
+        ctrl->chunk[slot] = s_chunk;
+    }
+    __syncthreads();
+    const long long span = (long long)WARP * s_chunk;
+    long long s = 0;
+    for (long long j = j0; j < j1; ++j) s += ((long long)task_hi[j] - (same ? j : 0) + span - 1) / span;
+    __syncthreads();
+    part[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = 1; o < 1024; o <<= 1) {
+        long long v = ((int)threadIdx.x >= o) ? part[threadIdx.x - o] : 0;
+        __syncthreads();
+        part[threadIdx.x] += v;
+        __syncthreads();
+    }
+    long long run = part[threadIdx.x] - s;
+    for (long long j = j0; j < j1; ++j) { tile_start[j] = run; run += ((long long)task_hi[j] - (same ? j : 0) + span - 1) / span; }
+    if (threadIdx.x == blockDim.x - 1) { tile_start[nk] = part[threadIdx.x]; ctrl->ntiles[slot] = (unsigned long long)part[threadIdx.x]; }
+}
+
+}  // namespace te

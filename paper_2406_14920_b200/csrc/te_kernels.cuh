@@ -223,6 +223,7 @@ struct JKArgs {
     const double* Ds; const double* Dm; double* Jt; double* Kt;
     const double* boys_tab;
     const long long* tile_start;
+    const int* task_hi;
     JKControl* ctrl;
     double tau;
     int nbf, nshells, slot, same;

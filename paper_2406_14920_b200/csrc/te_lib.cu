@@ -245,8 +245,9 @@ extern "C" int te_shellpair_build(const te_basis* b, double tau_pair, te_pairs**
         set_error("te_shellpair_build: scratch allocation failed"); te_pairs_destroy(P); return TE_ERR_ALLOC;
     }
     long long maxtiles = 0;
-    for (int c = 0; c < TE_NCLASS; ++c) maxtiles = std::max(maxtiles, P->count[c] / 4 + 2);
-    if (cudaMalloc(&P->d_tile_start, (maxtiles + 1) * sizeof(long long)) != cudaSuccess) {
+    for (int c = 0; c < TE_NCLASS; ++c) maxtiles = std::max(maxtiles, P->count[c] + 2);
+    if (cudaMalloc(&P->d_tile_start, (maxtiles + 1) * sizeof(long long)) != cudaSuccess ||
+        cudaMalloc(&P->d_task_hi, (maxtiles + 1) * sizeof(int)) != cudaSuccess) {
         set_error("te_shellpair_build: scratch allocation failed"); te_pairs_destroy(P); return TE_ERR_ALLOC;
     }
     P->tile_cap = maxtiles;
@@ -258,7 +259,7 @@ extern "C" int te_shellpair_build(const te_basis* b, double tau_pair, te_pairs**
 extern "C" void te_pairs_destroy(te_pairs* P) {
     if (!P) return;
     for (int c = 0; c < TE_NCLASS; ++c) { cudaFree(P->d_pair[c]); cudaFree(P->d_q[c]); cudaFree(P->d_ids[c]); }
-    cudaFree(P->d_Ds); cudaFree(P->d_Jt); cudaFree(P->d_Kt); cudaFree(P->d_Dm); cudaFree(P->d_ctrl); cudaFree(P->d_tile_start);
+    cudaFree(P->d_Ds); cudaFree(P->d_Jt); cudaFree(P->d_Kt); cudaFree(P->d_Dm); cudaFree(P->d_ctrl); cudaFree(P->d_tile_start); cudaFree(P->d_task_hi);
     cudaFree(P->d_hD); cudaFree(P->d_hJ); cudaFree(P->d_hK);
     for (int i = 0; i < TE_NCLASS * TE_NCLASS; ++i) { if (P->ev0[i]) cudaEventDestroy(P->ev0[i]); if (P->ev1[i]) cudaEventDestroy(P->ev1[i]); }
     delete P;
@@ -358,6 +359,7 @@ extern "C" int te_build_jk(const te_pairs* Pc, const double* D, double* J, doubl
     density_bounds_kernel<<<592, 256, 0, st>>>(D, b->d_shell_off, b->nshells, nbf, P->d_Dm, P->d_ctrl);
     int rc = TE_OK;
     const char* only = getenv("TE_DEBUG_SLOT");   // debugging aid: run a single class pair "cb*10+ck"
+    for (int i = 0; i < TE_NCLASS * TE_NCLASS; ++i) P->ev_valid[i] = false;
     for (int cb = 0; cb < TE_NCLASS && rc == TE_OK; ++cb)
         for (int ck = cb; ck < TE_NCLASS && rc == TE_OK; ++ck) {
             if (P->count[cb] == 0 || P->count[ck] == 0) continue;
@@ -365,7 +367,7 @@ extern "C" int te_build_jk(const te_pairs* Pc, const double* D, double* J, doubl
             const int slot = cb * TE_NCLASS + ck;
             if (P->profiling) cudaEventRecord(P->ev0[slot], st);
             rc = launch_jk_class(cb, ck, P, tau, st);
-            if (P->profiling) cudaEventRecord(P->ev1[slot], st);
+            if (P->profiling) { cudaEventRecord(P->ev1[slot], st); P->ev_valid[slot] = true; }
         }
     if (rc != TE_OK) return rc;
     finish_kernel<<<592, 256, 0, st>>>(P->d_Jt, P->d_Kt, b->d_aofac, nbf, J, K);
@@ -408,7 +410,7 @@ extern "C" int te_jk_stats(const te_pairs* P, long long quartets[TE_NCLASS][TE_N
             if (quartets) quartets[cb][ck] = (long long)h.live[slot];
             if (ms) {
                 float t = 0.f;
-                if (P->profiling && ck >= cb && P->count[cb] && P->count[ck]) cudaEventElapsedTime(&t, P->ev0[slot], P->ev1[slot]);
+                if (P->ev_valid[slot]) cudaEventElapsedTime(&t, P->ev0[slot], P->ev1[slot]);
                 ms[cb][ck] = t;
             }
         }
