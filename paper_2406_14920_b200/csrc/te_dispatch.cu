@@ -7,7 +7,7 @@ namespace te {
 #define TE_DECL(n)                                                                                         \
     int launch_schwarz_cb##n(const te_basis*, long long, double*, long long*);                             \
     int launch_pair_fill_cb##n(const te_basis*, long long, const long long*, PairD*, PairIds*);            \
-    int launch_jk_cb##n(int, te_pairs*, double, cudaStream_t);                                             \
+    int launch_jk_cb##n(int, te_pairs*, double, int, cudaStream_t);                                             \
     int launch_eri_cb##n(int, const te_basis*, int, const EriTask*, double*);
 TE_FOR_CLASSES(TE_DECL)
 
@@ -30,9 +30,9 @@ int launch_pair_fill(int la, int lb, const te_basis* b, long long n, const long 
     return TE_ERR_BAD_ARG;
 }
 
-int launch_jk_class(int cb, int ck, te_pairs* P, double tau, cudaStream_t st) {
+int launch_jk_class(int cb, int ck, te_pairs* P, double tau, int lane, cudaStream_t st) {
     switch (cb) {
-#define TE_CASE(n) case n: return launch_jk_cb##n(ck, P, tau, st);
+#define TE_CASE(n) case n: return launch_jk_cb##n(ck, P, tau, lane, st);
         TE_FOR_CLASSES(TE_CASE)
 #undef TE_CASE
     }

@@ -35,7 +35,7 @@ int TE_CAT(launch_pair_fill_cb, TE_CB)(const te_basis* b, long long n, const lon
 }
 
 template <int CK>
-static int jk_launch(te_pairs* P, double tau, cudaStream_t st) {
+static int jk_launch(te_pairs* P, double tau, int lane, cudaStream_t st) {
     constexpr int LC = CLS_LA[CK], LD = CLS_LB[CK];
     constexpr bool light = use_full_unroll(LA, LB, LC, LD);
     constexpr int TB = light ? 16 : 8, TK = light ? 16 : 8;
@@ -45,15 +45,15 @@ static int jk_launch(te_pairs* P, double tau, cudaStream_t st) {
     a.pb = P->d_pair[TE_CB]; a.qb = P->d_q[TE_CB]; a.ib = P->d_ids[TE_CB]; a.nb = P->count[TE_CB];
     a.pk = P->d_pair[CK]; a.qk = P->d_q[CK]; a.ik = P->d_ids[CK]; a.nk = P->count[CK];
     a.Ds = P->d_Ds; a.Dm = P->d_Dm; a.Jt = P->d_Jt; a.Kt = P->d_Kt; a.boys_tab = b->d_boys;
-    a.tile_start = P->d_tile_start; a.ctrl = P->d_ctrl; a.tau = tau; a.nbf = b->nbf; a.nshells = b->nshells;
+    a.tile_start = P->d_tile_start[lane]; a.ctrl = P->d_ctrl; a.tau = tau; a.nbf = b->nbf; a.nshells = b->nshells;
     a.slot = slot; a.same = (TE_CB == CK);
-    a.task_hi = P->d_task_hi;
+    a.task_hi = P->d_task_hi[lane];
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     static const int impl = getenv("TE_JK_IMPL") ? atoi(getenv("TE_JK_IMPL")) : 1;   // 0: generic thread-per-quartet kernel everywhere
     if (light || impl == 0) {
-        schedule_kernel<<<1, 1024, 0, st>>>(a.qb, a.nb, a.qk, a.nk, a.same, tau, TB, TK, P->d_tile_start, P->d_ctrl, slot);
+        schedule_kernel<<<1, 1024, 0, st>>>(a.qb, a.nb, a.qk, a.nk, a.same, tau, TB, TK, P->d_tile_start[lane], P->d_ctrl, slot);
         const long long max_tiles = ((a.nb + TB - 1) / TB) * ((a.nk + TK - 1) / TK);
         const int per_sm = light ? 8 : 16;   // resident CTAs per SM worth of persistent blocks
         const unsigned grid = (unsigned)std::min<long long>(max_tiles, (long long)sms * per_sm);
@@ -69,7 +69,7 @@ static int jk_launch(te_pairs* P, double tau, cudaStream_t st) {
             if (blocks_per_sm < 1) { set_error("jkw_kernel<%d,%d,%d,%d>: %d bytes of shared memory do not fit", LA, LB, LC, LD, smem); blocks_per_sm = 0; return TE_ERR_CUDA; }
         }
         const int warps = sms * blocks_per_sm;
-        schedule_w_kernel<<<1, 1024, 0, st>>>(a.qb, a.nb, a.qk, a.nk, a.same, tau, warps, P->d_tile_start, P->d_task_hi, P->d_ctrl, slot);
+        schedule_w_kernel<<<1, 1024, 0, st>>>(a.qb, a.nb, a.qk, a.nk, a.same, tau, warps, P->d_tile_start[lane], P->d_task_hi[lane], P->d_ctrl, slot);
         const long long max_tasks = a.nk * ((a.nb + WARP - 1) / WARP);
         const unsigned grid = (unsigned)std::min<long long>(max_tasks, (long long)warps);
         jkw_kernel<LA, LB, LC, LD><<<grid, WARP, smem, st>>>(a);
@@ -87,9 +87,9 @@ static int eri_launch(const te_basis* b, int n, const EriTask* d_tasks, double* 
 }
 
 template <int CK>
-static int jk_dispatch(int ck, te_pairs* P, double tau, cudaStream_t st) {
-    if (ck == CK) return jk_launch<CK>(P, tau, st);
-    if constexpr (CK + 1 < TE_NCLASS) return jk_dispatch<CK + 1>(ck, P, tau, st);
+static int jk_dispatch(int ck, te_pairs* P, double tau, int lane, cudaStream_t st) {
+    if (ck == CK) return jk_launch<CK>(P, tau, lane, st);
+    if constexpr (CK + 1 < TE_NCLASS) return jk_dispatch<CK + 1>(ck, P, tau, lane, st);
     set_error("launch_jk: bad ket class %d", ck);
     return TE_ERR_BAD_ARG;
 }
@@ -102,7 +102,7 @@ static int eri_dispatch(int ck, const te_basis* b, int n, const EriTask* d_tasks
     return TE_ERR_BAD_ARG;
 }
 
-int TE_CAT(launch_jk_cb, TE_CB)(int ck, te_pairs* P, double tau, cudaStream_t st) { return jk_dispatch<TE_CB>(ck, P, tau, st); }
+int TE_CAT(launch_jk_cb, TE_CB)(int ck, te_pairs* P, double tau, int lane, cudaStream_t st) { return jk_dispatch<TE_CB>(ck, P, tau, lane, st); }
 int TE_CAT(launch_eri_cb, TE_CB)(int ck, const te_basis* b, int n, const EriTask* d_tasks, double* out_dev) {
     return eri_dispatch<TE_CB>(ck, b, n, d_tasks, out_dev);
 }

@@ -64,8 +64,13 @@ struct te_pairs {
     // per-build scratch
     double *d_Ds = nullptr, *d_Jt = nullptr, *d_Kt = nullptr, *d_Dm = nullptr;
     te::JKControl* d_ctrl = nullptr;
-    long long* d_tile_start = nullptr;
-    int* d_task_hi = nullptr;
+    // class-pair kernels of one build run concurrently on NSTREAM internal streams (forked from / joined to the
+    // caller's stream with events); each internal stream owns its schedule scratch
+    static constexpr int NSTREAM = 8;
+    cudaStream_t streams[NSTREAM] = {nullptr};
+    cudaEvent_t ev_fork = nullptr, ev_join[NSTREAM] = {nullptr};
+    long long* d_tile_start[NSTREAM] = {nullptr};
+    int* d_task_hi[NSTREAM] = {nullptr};
     long long tile_cap = 0;
     double *d_hD = nullptr, *d_hJ = nullptr, *d_hK = nullptr;   // staging for te_build_jk_host
     bool profiling = false;
@@ -78,6 +83,6 @@ namespace te {
 // te_inst_*.cu
 int launch_schwarz(int la, int lb, const te_basis* b, long long ncand, double* d_q, long long* d_idx);
 int launch_pair_fill(int la, int lb, const te_basis* b, long long n, const long long* d_idx, PairD* d_pair, PairIds* d_ids);
-int launch_jk_class(int cb, int ck, te_pairs* P, double tau, cudaStream_t st);
+int launch_jk_class(int cb, int ck, te_pairs* P, double tau, int lane, cudaStream_t st);   // lane: which schedule scratch
 int launch_eri_class(int cb, int ck, const te_basis* b, int n, const EriTask* d_tasks, double* out_dev);
 }  // namespace te

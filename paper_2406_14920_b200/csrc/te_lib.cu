@@ -67,6 +67,9 @@ static int upload(const std::vector<T>& h, T** d) {
     return TE_OK;
 }
 
+static const int CLS_LA_H[TE_NCLASS] = {0, 0, 0, 0, 1, 1, 1, 2, 2, 3};
+static const int CLS_LB_H[TE_NCLASS] = {0, 1, 2, 3, 1, 2, 3, 2, 3, 3};
+
 static double dfact(int n) { double r = 1.0; for (; n > 1; n -= 2) r *= n; return r; }
 
 }  // namespace te
@@ -246,9 +249,16 @@ extern "C" int te_shellpair_build(const te_basis* b, double tau_pair, te_pairs**
     }
     long long maxtiles = 0;
     for (int c = 0; c < TE_NCLASS; ++c) maxtiles = std::max(maxtiles, P->count[c] + 2);
-    if (cudaMalloc(&P->d_tile_start, (maxtiles + 1) * sizeof(long long)) != cudaSuccess ||
-        cudaMalloc(&P->d_task_hi, (maxtiles + 1) * sizeof(int)) != cudaSuccess) {
-        set_error("te_shellpair_build: scratch allocation failed"); te_pairs_destroy(P); return TE_ERR_ALLOC;
+    for (int s = 0; s < te_pairs::NSTREAM; ++s) {
+        if (cudaMalloc(&P->d_tile_start[s], (maxtiles + 1) * sizeof(long long)) != cudaSuccess ||
+            cudaMalloc(&P->d_task_hi[s], (maxtiles + 1) * sizeof(int)) != cudaSuccess ||
+            cudaStreamCreateWithFlags(&P->streams[s], cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&P->ev_join[s], cudaEventDisableTiming) != cudaSuccess) {
+            set_error("te_shellpair_build: scratch allocation failed"); te_pairs_destroy(P); return TE_ERR_ALLOC;
+        }
+    }
+    if (cudaEventCreateWithFlags(&P->ev_fork, cudaEventDisableTiming) != cudaSuccess) {
+        set_error("te_shellpair_build: event creation failed"); te_pairs_destroy(P); return TE_ERR_ALLOC;
     }
     P->tile_cap = maxtiles;
     for (int i = 0; i < TE_NCLASS * TE_NCLASS; ++i) { cudaEventCreate(&P->ev0[i]); cudaEventCreate(&P->ev1[i]); }
@@ -259,7 +269,13 @@ extern "C" int te_shellpair_build(const te_basis* b, double tau_pair, te_pairs**
 extern "C" void te_pairs_destroy(te_pairs* P) {
     if (!P) return;
     for (int c = 0; c < TE_NCLASS; ++c) { cudaFree(P->d_pair[c]); cudaFree(P->d_q[c]); cudaFree(P->d_ids[c]); }
-    cudaFree(P->d_Ds); cudaFree(P->d_Jt); cudaFree(P->d_Kt); cudaFree(P->d_Dm); cudaFree(P->d_ctrl); cudaFree(P->d_tile_start); cudaFree(P->d_task_hi);
+    cudaFree(P->d_Ds); cudaFree(P->d_Jt); cudaFree(P->d_Kt); cudaFree(P->d_Dm); cudaFree(P->d_ctrl);
+    for (int s = 0; s < te_pairs::NSTREAM; ++s) {
+        cudaFree(P->d_tile_start[s]); cudaFree(P->d_task_hi[s]);
+        if (P->streams[s]) cudaStreamDestroy(P->streams[s]);
+        if (P->ev_join[s]) cudaEventDestroy(P->ev_join[s]);
+    }
+    if (P->ev_fork) cudaEventDestroy(P->ev_fork);
     cudaFree(P->d_hD); cudaFree(P->d_hJ); cudaFree(P->d_hK);
     for (int i = 0; i < TE_NCLASS * TE_NCLASS; ++i) { if (P->ev0[i]) cudaEventDestroy(P->ev0[i]); if (P->ev1[i]) cudaEventDestroy(P->ev1[i]); }
     delete P;
@@ -360,15 +376,39 @@ extern "C" int te_build_jk(const te_pairs* Pc, const double* D, double* J, doubl
     int rc = TE_OK;
     const char* only = getenv("TE_DEBUG_SLOT");   // debugging aid: run a single class pair "cb*10+ck"
     for (int i = 0; i < TE_NCLASS * TE_NCLASS; ++i) P->ev_valid[i] = false;
-    for (int cb = 0; cb < TE_NCLASS && rc == TE_OK; ++cb)
-        for (int ck = cb; ck < TE_NCLASS && rc == TE_OK; ++ck) {
+    // class pairs, most expensive first (pair counts x transform work of one quartet), so the long kernels start early
+    struct Job { int cb, ck; double w; };
+    std::vector<Job> jobs;
+    for (int cb = 0; cb < TE_NCLASS; ++cb)
+        for (int ck = cb; ck < TE_NCLASS; ++ck) {
             if (P->count[cb] == 0 || P->count[ck] == 0) continue;
             if (only && atoi(only) != cb * TE_NCLASS + ck) continue;
-            const int slot = cb * TE_NCLASS + ck;
-            if (P->profiling) cudaEventRecord(P->ev0[slot], st);
-            rc = launch_jk_class(cb, ck, P, tau, st);
-            if (P->profiling) { cudaEventRecord(P->ev1[slot], st); P->ev_valid[slot] = true; }
+            const int la = CLS_LA_H[cb], lb = CLS_LB_H[cb], lc = CLS_LA_H[ck], ld = CLS_LB_H[ck];
+            const double w = (double)P->count[cb] * (double)P->count[ck] *
+                             (60.0 + nherm(la + lb) * (double)nherm(lc + ld) + 7.0 * ncart(la) * ncart(lb) * ncart(lc) * ncart(ld));
+            jobs.push_back(Job{cb, ck, w});
         }
+    std::sort(jobs.begin(), jobs.end(), [](const Job& x, const Job& y) { return x.w > y.w; });
+    if (P->profiling) {
+        // serial, on the caller's stream, with an event pair around every class pair
+        for (const Job& j : jobs) {
+            const int slot = j.cb * TE_NCLASS + j.ck;
+            cudaEventRecord(P->ev0[slot], st);
+            if ((rc = launch_jk_class(j.cb, j.ck, P, tau, 0, st)) != TE_OK) return rc;
+            cudaEventRecord(P->ev1[slot], st);
+            P->ev_valid[slot] = true;
+        }
+    } else {
+        // fork: every internal stream waits for the preamble on the caller's stream; join: the caller's stream waits for all
+        constexpr int NS = te_pairs::NSTREAM;
+        TE_CUDA(cudaEventRecord(P->ev_fork, st));
+        for (int s = 0; s < NS; ++s) TE_CUDA(cudaStreamWaitEvent(P->streams[s], P->ev_fork, 0));
+        for (size_t i = 0; i < jobs.size() && rc == TE_OK; ++i) rc = launch_jk_class(jobs[i].cb, jobs[i].ck, P, tau, (int)(i % NS), P->streams[i % NS]);
+        for (int s = 0; s < NS; ++s) {
+            TE_CUDA(cudaEventRecord(P->ev_join[s], P->streams[s]));
+            TE_CUDA(cudaStreamWaitEvent(st, P->ev_join[s], 0));
+        }
+    }
     if (rc != TE_OK) return rc;
     finish_kernel<<<592, 256, 0, st>>>(P->d_Jt, P->d_Kt, b->d_aofac, nbf, J, K);
     TE_CUDA(cudaGetLastError());
