@@ -69,8 +69,8 @@ static int jk_launch(te_pairs* P, double tau, int lane, cudaStream_t st) {
             if (blocks_per_sm < 1) { set_error("jkw_kernel<%d,%d,%d,%d>: %d bytes of shared memory do not fit", LA, LB, LC, LD, smem); blocks_per_sm = 0; return TE_ERR_CUDA; }
         }
         const int warps = sms * blocks_per_sm;
-        schedule_w_kernel<<<1, 1024, 0, st>>>(a.qb, a.nb, a.qk, a.nk, a.same, tau, warps, P->d_tile_start[lane], P->d_task_hi[lane], P->d_ctrl, slot);
-        const long long max_tasks = a.nk * ((a.nb + WARP - 1) / WARP);
+        schedule_w_kernel<<<1, 1024, 0, st>>>(a.qb, a.nb, a.qk, a.nk, a.same, tau, warps, S::NL, P->d_tile_start[lane], P->d_task_hi[lane], P->d_ctrl, slot);
+        const long long max_tasks = a.nk * ((a.nb + S::NL - 1) / S::NL);
         const unsigned grid = (unsigned)std::min<long long>(max_tasks, (long long)warps);
         jkw_kernel<LA, LB, LC, LD><<<grid, WARP, smem, st>>>(a);
     }

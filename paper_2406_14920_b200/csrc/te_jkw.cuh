@@ -38,11 +38,15 @@ struct WShape {
     static constexpr int NE1 = (LC + 1) * (LD + 1) * (LCD + 1);
     // K_?c accumulators / D_?c blocks of the smaller ket shell stay in registers for the whole quartet when small
     static constexpr bool KEEPC = (NA + NB) * NC <= 24;
-    static constexpr int smem_doubles = NR * WARP + NNZK + 3 * NE1 + NC * ND;
+    // NL = lanes of the warp that hold a quartet (R column stride).  Measured on B200: narrowing the warp to 8 lanes for L >= 10
+    // (4x more resident warps) made (DF|DF) 2.4x SLOWER -- these kernels are bound by per-warp instruction / local-memory
+    // throughput, not by latency -- so every lane holds a quartet.
+    static constexpr int NL = 32;
+    static constexpr int smem_doubles = NR * NL + NNZK + 3 * NE1 + NC * ND;
 };
 
 // R^0_{tuv} of eq. 21-25 built in place in a shared-memory column (element i at R[i * 32]); same sweep as rtable<L>.
-template <int L>
+template <int L, int RS>
 __device__ __forceinline__ void rtable_sm(double alpha, double X, double Y, double Z, const double* __restrict__ F, double* R) {
     double fac[L + 1];
     fac[0] = 1.0;
@@ -60,16 +64,16 @@ __device__ __forceinline__ void rtable_sm(double alpha, double X, double Y, doub
                     const int v = n - t - u;
                     double r;
                     if (t > 0) {
-                        r = X * R[tidx<L>(t - 1, u, v) * WARP];
-                        if (t > 1) r = fma((double)(t - 1), R[tidx<L>(t - 2, u, v) * WARP], r);
+                        r = X * R[tidx<L>(t - 1, u, v) * RS];
+                        if (t > 1) r = fma((double)(t - 1), R[tidx<L>(t - 2, u, v) * RS], r);
                     } else if (u > 0) {
-                        r = Y * R[tidx<L>(t, u - 1, v) * WARP];
-                        if (u > 1) r = fma((double)(u - 1), R[tidx<L>(t, u - 2, v) * WARP], r);
+                        r = Y * R[tidx<L>(t, u - 1, v) * RS];
+                        if (u > 1) r = fma((double)(u - 1), R[tidx<L>(t, u - 2, v) * RS], r);
                     } else {
-                        r = Z * R[tidx<L>(t, u, v - 1) * WARP];
-                        if (v > 1) r = fma((double)(v - 1), R[tidx<L>(t, u, v - 2) * WARP], r);
+                        r = Z * R[tidx<L>(t, u, v - 1) * RS];
+                        if (v > 1) r = fma((double)(v - 1), R[tidx<L>(t, u, v - 2) * RS], r);
                     }
-                    R[tidx<L>(t, u, v) * WARP] = r;
+                    R[tidx<L>(t, u, v) * RS] = r;
                 }
             }
         }
@@ -83,18 +87,19 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
     constexpr int LAB = S::LAB, LCD = S::LCD, L = S::L;
     constexpr int NA = S::NA, NB = S::NB, NC = S::NC, ND = S::ND, NHB = S::NHB;
     constexpr bool KEEPC = S::KEEPC;
+    constexpr int NL = S::NL;
     constexpr unsigned FULLMASK = 0xffffffffu;
     extern __shared__ double sm[];
     double* const Rsm = sm;
-    double* const kt = Rsm + S::NR * WARP;
+    double* const kt = Rsm + S::NR * NL;
     double* const e1 = kt + S::NNZK;
     double* const dcd = e1 + 3 * S::NE1;
     const int lane = threadIdx.x;
-    double* const Rl = Rsm + lane;
+    double* const Rl = Rsm + (lane < NL ? lane : 0);   // lanes >= NL never hold a quartet
     const unsigned short* const rowtab = c_rowtab.v + L * 169;
 
     const unsigned long long ntasks = a.ctrl->ntiles[a.slot];
-    const long long span = (long long)WARP * a.ctrl->chunk[a.slot];
+    const long long span = (long long)NL * a.ctrl->chunk[a.slot];
     const long long ns = a.nshells;
     const long long nbf = a.nbf;
     long long cached_j = -1;
@@ -150,9 +155,9 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
             cached_j = j;
         }
 
-        for (long long b0 = b_lo; b0 < b_hi; b0 += WARP) {
+        for (long long b0 = b_lo; b0 < b_hi; b0 += NL) {
             const long long bi = b0 + lane;
-            bool active = bi < b_hi;
+            bool active = lane < NL && bi < b_hi;
             PairD bp;
             PairIds ib;
             bool live_jab = false, live_jcd = false, live_kac = false, live_kbc = false, live_kad = false, live_kbd = false;
@@ -189,7 +194,7 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                 const double pref = 34.986836655249725693 / (p * q * sqrt(pq)) * bp.pref * f;
 #pragma unroll
                 for (int m = 0; m <= L; ++m) F[m] *= pref;
-                rtable_sm<L>(alpha, X, Y, Z, F, Rl);
+                rtable_sm<L, NL>(alpha, X, Y, Z, F, Rl);
                 const double hb = 0.5 / p;
                 etable<LA, LB, false>(bp.PA[0], bp.PB[0], hb, Ebx);
                 etable<LA, LB, false>(bp.PA[1], bp.PB[1], hb, Eby);
@@ -234,15 +239,15 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                                 const unsigned short* rt = rowtab + t2 * 13 + u2;
                                 for (int v2 = 0; v2 <= sz; ++v2) {
                                     const double e = *ktp++;
-                                    const double* Rq = Rl + v2 * WARP;
+                                    const double* Rq = Rl + v2 * NL;
 #pragma unroll
                                     for (int t = 0; t <= LAB; ++t)
 #pragma unroll
                                         for (int u = 0; u <= LAB - t; ++u) {
-                                            const double* Rrow = Rq + (int)rt[t * 13 + u] * WARP;
+                                            const double* Rrow = Rq + (int)rt[t * 13 + u] * NL;
 #pragma unroll
                                             for (int v = 0; v <= LAB - t - u; ++v)
-                                                Yv[tidx<LAB>(t, u, v)] = fma(e, Rrow[v * WARP], Yv[tidx<LAB>(t, u, v)]);
+                                                Yv[tidx<LAB>(t, u, v)] = fma(e, Rrow[v * NL], Yv[tidx<LAB>(t, u, v)]);
                                         }
                                 }
                             }
@@ -354,7 +359,7 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
 // [same ? j : 0, cut_j) with cut_j = first bra whose q_bra * q_ket[j] * max|D| < tau (eq. 47, loosest density bound); a task is
 // (ket j, chunk of 32*chunk bras).  task_hi[j] = cut_j, tile_start = exclusive prefix sum of the chunk counts.
 static __global__ void __launch_bounds__(1024) schedule_w_kernel(const double* __restrict__ qb, long long nb, const double* __restrict__ qk,
-                                                          long long nk, int same, double tau, int target_warps,
+                                                          long long nk, int same, double tau, int target_warps, int lanes,
                                                           long long* __restrict__ tile_start, int* __restrict__ task_hi, JKControl* ctrl, int slot) {
     __shared__ long long part[1024];
     __shared__ int s_chunk;
@@ -388,12 +393,12 @@ static __global__ void __launch_bounds__(1024) schedule_w_kernel(const double* _
     }
     if (threadIdx.x == 0) {
         // chunk: 32*chunk bras per task, sized so every resident warp gets ~8 tasks; 1..16
-        long long c = part[0] / ((long long)WARP * target_warps * 8);
+        long long c = part[0] / ((long long)lanes * target_warps * 8);
         s_chunk = (int)max(1LL, min(16LL, c));
         ctrl->chunk[slot] = s_chunk;
     }
     __syncthreads();
-    const long long span = (long long)WARP * s_chunk;
+    const long long span = (long long)lanes * s_chunk;
     long long s = 0;
     for (long long j = j0; j < j1; ++j) s += ((long long)task_hi[j] - (same ? j : 0) + span - 1) / span;
     __syncthreads();

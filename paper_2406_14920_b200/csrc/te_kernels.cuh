@@ -230,7 +230,7 @@ struct JKArgs {
 };
 
 template <int LA, int LB, int LC, int LD, int TB, int TK>
-__global__ void __launch_bounds__(TB * TK, 1) jk_kernel(JKArgs a) {
+__global__ void __launch_bounds__(TB * TK, (TB * TK >= 256 ? 2 : 1)) jk_kernel(JKArgs a) {
     constexpr bool FULL = use_full_unroll(LA, LB, LC, LD);
     __shared__ unsigned int s_tile;
     const long long nbt = (a.nb + TB - 1) / TB;
