@@ -8,7 +8,9 @@ namespace te {
     int launch_schwarz_cb##n(const te_basis*, long long, double*, long long*);                             \
     int launch_pair_fill_cb##n(const te_basis*, long long, const long long*, PairD*, PairIds*);            \
     int launch_jk_cb##n(int, te_pairs*, double, int, cudaStream_t);                                             \
-    int launch_eri_cb##n(int, const te_basis*, int, const EriTask*, double*);
+    int launch_eri_cb##n(int, const te_basis*, int, const EriTask*, double*);                              \
+    int launch_hermite_density_cb##n(te_pairs*, cudaStream_t);                                             \
+    int launch_hermite_j_cb##n(te_pairs*, cudaStream_t);
 TE_FOR_CLASSES(TE_DECL)
 
 int launch_schwarz(int la, int lb, const te_basis* b, long long ncand, double* d_q, long long* d_idx) {
@@ -42,6 +44,24 @@ int launch_jk_class(int cb, int ck, te_pairs* P, double tau, int lane, cudaStrea
 int launch_eri_class(int cb, int ck, const te_basis* b, int n, const EriTask* d_tasks, double* out_dev) {
     switch (cb) {
 #define TE_CASE(k) case k: return launch_eri_cb##k(ck, b, n, d_tasks, out_dev);
+        TE_FOR_CLASSES(TE_CASE)
+#undef TE_CASE
+    }
+    return TE_ERR_BAD_ARG;
+}
+
+int launch_hermite_density(int cls, te_pairs* P, cudaStream_t st) {
+    switch (cls) {
+#define TE_CASE(k) case k: return launch_hermite_density_cb##k(P, st);
+        TE_FOR_CLASSES(TE_CASE)
+#undef TE_CASE
+    }
+    return TE_ERR_BAD_ARG;
+}
+
+int launch_hermite_j(int cls, te_pairs* P, cudaStream_t st) {
+    switch (cls) {
+#define TE_CASE(k) case k: return launch_hermite_j_cb##k(P, st);
         TE_FOR_CLASSES(TE_CASE)
 #undef TE_CASE
     }

@@ -1,6 +1,6 @@
 // te_inst.cu -- instantiates every kernel whose BRA pair class is TE_CB (compiled 10 times, -DTE_CB=0..9, so the
 // 55 (la lb|lc ld) classes build in parallel).  Exposes launch_*_cb<TE_CB> entry points used by te_dispatch.cu.
-#include "te_jkw.cuh"
+#include "te_jkq.cuh"
 
 #include <cstdlib>
 
@@ -51,7 +51,36 @@ static int jk_launch(te_pairs* P, double tau, int lane, cudaStream_t st) {
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    static const int impl = getenv("TE_JK_IMPL") ? atoi(getenv("TE_JK_IMPL")) : 1;   // 0: generic thread-per-quartet kernel everywhere
+    // 0: generic thread-per-quartet kernel everywhere; 1: uniform-ket warp kernel for the non-light classes;
+    // 2 (default): split-quartet kernel where instantiated (use_jkq), uniform-ket warp kernel otherwise
+    static const int impl = getenv("TE_JK_IMPL") ? atoi(getenv("TE_JK_IMPL")) : 2;
+    if constexpr (use_jkq(LA, LB, LC, LD)) {
+        if (impl == 2) {
+            constexpr int QW = 4, QG = jkq_lanes(LA, LB, LC, LD, QW);
+            using S = QShape<LA, LB, LC, LD, QG, QW>;
+            using Tab = QTab<LA, LB, LC, LD>;
+            static Tab* d_tab = nullptr;
+            static int blocks_per_sm = 0;
+            if (!d_tab) {
+                static const Tab h_tab;
+                Tab* d = nullptr;
+                TE_CUDA(cudaMalloc(&d, sizeof(Tab)));
+                TE_CUDA(cudaMemcpy(d, &h_tab, sizeof(Tab), cudaMemcpyHostToDevice));
+                TE_CUDA(cudaFuncSetAttribute(jkq_kernel<LA, LB, LC, LD, QG, QW>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::smem_bytes));
+                TE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, jkq_kernel<LA, LB, LC, LD, QG, QW>, 32 * QW, S::smem_bytes));
+                if (blocks_per_sm < 1) { cudaFree(d); set_error("jkq_kernel<%d,%d,%d,%d>: %d bytes of shared memory do not fit", LA, LB, LC, LD, S::smem_bytes); return TE_ERR_CUDA; }
+                d_tab = d;
+            }
+            a.DHb = P->d_DH[TE_CB]; a.DHk = P->d_DH[CK]; a.JHb = P->d_JH[TE_CB]; a.JHk = P->d_JH[CK];
+            const int blocks = sms * blocks_per_sm;
+            schedule_w_kernel<<<1, 1024, 0, st>>>(a.qb, a.nb, a.qk, a.nk, a.same, tau, blocks, S::NQ * QW, P->d_tile_start[lane], P->d_task_hi[lane], P->d_ctrl, slot);
+            const long long max_tasks = a.nk * ((a.nb + S::NQ * QW - 1) / (S::NQ * QW));
+            const unsigned grid = (unsigned)std::min<long long>(max_tasks, (long long)blocks);
+            jkq_kernel<LA, LB, LC, LD, QG, QW><<<grid, 32 * QW, S::smem_bytes, st>>>(a, d_tab);
+            TE_CUDA(cudaGetLastError());
+            return TE_OK;
+        }
+    }
     if (light || impl == 0) {
         schedule_kernel<<<1, 1024, 0, st>>>(a.qb, a.nb, a.qk, a.nk, a.same, tau, TB, TK, P->d_tile_start[lane], P->d_ctrl, slot);
         const long long max_tiles = ((a.nb + TB - 1) / TB) * ((a.nk + TK - 1) / TK);
@@ -74,6 +103,22 @@ static int jk_launch(te_pairs* P, double tau, int lane, cudaStream_t st) {
         const unsigned grid = (unsigned)std::min<long long>(max_tasks, (long long)warps);
         jkw_kernel<LA, LB, LC, LD><<<grid, WARP, smem, st>>>(a);
     }
+    TE_CUDA(cudaGetLastError());
+    return TE_OK;
+}
+
+int TE_CAT(launch_hermite_density_cb, TE_CB)(te_pairs* P, cudaStream_t st) {
+    const long long n = P->count[TE_CB];
+    if (n == 0) return TE_OK;
+    hermite_density_kernel<LA, LB><<<(unsigned)((n + 127) / 128), 128, 0, st>>>(P->d_pair[TE_CB], P->d_ids[TE_CB], n, P->d_Ds, P->basis->nbf, P->d_DH[TE_CB]);
+    TE_CUDA(cudaGetLastError());
+    return TE_OK;
+}
+
+int TE_CAT(launch_hermite_j_cb, TE_CB)(te_pairs* P, cudaStream_t st) {
+    const long long n = P->count[TE_CB];
+    if (n == 0) return TE_OK;
+    hermite_j_kernel<LA, LB><<<(unsigned)((n + 127) / 128), 128, 0, st>>>(P->d_pair[TE_CB], P->d_ids[TE_CB], n, P->d_JH[TE_CB], P->basis->nbf, P->d_Jt);
     TE_CUDA(cudaGetLastError());
     return TE_OK;
 }

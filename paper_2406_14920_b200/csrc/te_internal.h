@@ -61,6 +61,9 @@ struct te_pairs {
     te::PairD* d_pair[TE_NCLASS] = {nullptr};
     double* d_q[TE_NCLASS] = {nullptr};
     te::PairIds* d_ids[TE_NCLASS] = {nullptr};
+    // Hermite density / Hermite J of every pair (eq. 35), [count][nherm(la+lb)], rebuilt / zeroed by every build
+    double* d_DH[TE_NCLASS] = {nullptr};
+    double* d_JH[TE_NCLASS] = {nullptr};
     // per-build scratch
     double *d_Ds = nullptr, *d_Jt = nullptr, *d_Kt = nullptr, *d_Dm = nullptr;
     te::JKControl* d_ctrl = nullptr;
@@ -85,4 +88,6 @@ int launch_schwarz(int la, int lb, const te_basis* b, long long ncand, double* d
 int launch_pair_fill(int la, int lb, const te_basis* b, long long n, const long long* d_idx, PairD* d_pair, PairIds* d_ids);
 int launch_jk_class(int cb, int ck, te_pairs* P, double tau, int lane, cudaStream_t st);   // lane: which schedule scratch
 int launch_eri_class(int cb, int ck, const te_basis* b, int n, const EriTask* d_tasks, double* out_dev);
+int launch_hermite_density(int cls, te_pairs* P, cudaStream_t st);   // d_Ds -> d_DH[cls]
+int launch_hermite_j(int cls, te_pairs* P, cudaStream_t st);         // d_JH[cls] -> d_Jt
 }  // namespace te

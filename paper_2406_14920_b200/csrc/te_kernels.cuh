@@ -222,6 +222,8 @@ struct JKArgs {
     const PairD* pk; const double* qk; const PairIds* ik; long long nk;
     const double* Ds; const double* Dm; double* Jt; double* Kt;
     const double* boys_tab;
+    const double* DHb; const double* DHk;   // Hermite densities of the bra / ket pair lists (split-quartet kernel)
+    double* JHb; double* JHk;               // Hermite J accumulators of the bra / ket pair lists
     const long long* tile_start;
     const int* task_hi;
     JKControl* ctrl;

@@ -232,6 +232,10 @@ extern "C" int te_shellpair_build(const te_basis* b, double tau_pair, te_pairs**
                     cudaMalloc(&P->d_ids[cls], nk * sizeof(PairIds)) != cudaSuccess) {
                     cleanup(); set_error("te_shellpair_build: pair allocation failed"); return fail(TE_ERR_ALLOC);
                 }
+                const size_t nh = (size_t)nk * nherm(la + lb) * sizeof(double);
+                if (cudaMalloc(&P->d_DH[cls], nh) != cudaSuccess || cudaMalloc(&P->d_JH[cls], nh) != cudaSuccess) {
+                    cleanup(); set_error("te_shellpair_build: Hermite buffer allocation failed"); return fail(TE_ERR_ALLOC);
+                }
                 cudaMemcpy(P->d_q[cls], d_qs, nk * sizeof(double), cudaMemcpyDeviceToDevice);
                 if ((rc = launch_pair_fill(la, lb, b, (long long)nk, d_idxs, P->d_pair[cls], P->d_ids[cls])) != TE_OK) { cleanup(); return fail(rc); }
             }
@@ -268,7 +272,7 @@ extern "C" int te_shellpair_build(const te_basis* b, double tau_pair, te_pairs**
 
 extern "C" void te_pairs_destroy(te_pairs* P) {
     if (!P) return;
-    for (int c = 0; c < TE_NCLASS; ++c) { cudaFree(P->d_pair[c]); cudaFree(P->d_q[c]); cudaFree(P->d_ids[c]); }
+    for (int c = 0; c < TE_NCLASS; ++c) { cudaFree(P->d_pair[c]); cudaFree(P->d_q[c]); cudaFree(P->d_ids[c]); cudaFree(P->d_DH[c]); cudaFree(P->d_JH[c]); }
     cudaFree(P->d_Ds); cudaFree(P->d_Jt); cudaFree(P->d_Kt); cudaFree(P->d_Dm); cudaFree(P->d_ctrl);
     for (int s = 0; s < te_pairs::NSTREAM; ++s) {
         cudaFree(P->d_tile_start[s]); cudaFree(P->d_task_hi[s]);
@@ -374,6 +378,12 @@ extern "C" int te_build_jk(const te_pairs* Pc, const double* D, double* J, doubl
     scale_density_kernel<<<592, 256, 0, st>>>(D, b->d_aofac, nbf, P->d_Ds);
     density_bounds_kernel<<<592, 256, 0, st>>>(D, b->d_shell_off, b->nshells, nbf, P->d_Dm, P->d_ctrl);
     int rc = TE_OK;
+    // Hermite density of every pair and zeroed Hermite J (eq. 35): inputs / accumulators of the split-quartet kernels
+    for (int c = 0; c < TE_NCLASS; ++c) {
+        if (P->count[c] == 0) continue;
+        TE_CUDA(cudaMemsetAsync(P->d_JH[c], 0, (size_t)P->count[c] * nherm(CLS_LA_H[c] + CLS_LB_H[c]) * sizeof(double), st));
+        if ((rc = launch_hermite_density(c, P, st)) != TE_OK) return rc;
+    }
     const char* only = getenv("TE_DEBUG_SLOT");   // debugging aid: run a single class pair "cb*10+ck"
     for (int i = 0; i < TE_NCLASS * TE_NCLASS; ++i) P->ev_valid[i] = false;
     // class pairs, most expensive first (pair counts x transform work of one quartet), so the long kernels start early
@@ -410,6 +420,9 @@ extern "C" int te_build_jk(const te_pairs* Pc, const double* D, double* J, doubl
         }
     }
     if (rc != TE_OK) return rc;
+    // Hermite J -> Cartesian J of every pair (the paper's CPU post-processing step, on the device)
+    for (int c = 0; c < TE_NCLASS; ++c)
+        if (P->count[c] && (rc = launch_hermite_j(c, P, st)) != TE_OK) return rc;
     finish_kernel<<<592, 256, 0, st>>>(P->d_Jt, P->d_Kt, b->d_aofac, nbf, J, K);
     TE_CUDA(cudaGetLastError());
     return TE_OK;
