@@ -46,8 +46,8 @@ def build(force: bool = False, jobs: int | None = None) -> str:
     os.makedirs(BUILD, exist_ok=True)
     work = [(os.path.join(CSRC, "te_lib.cu"), os.path.join(BUILD, "te_lib.o"), []),
             (os.path.join(CSRC, "te_dispatch.cu"), os.path.join(BUILD, "te_dispatch.o"), [])]
-    # heaviest bra classes first so the pool stays busy
-    for cb in (9, 8, 7, 6, 5, 4, 3, 2, 1, 0):
+    # slowest translation units first so the pool stays busy
+    for cb in (0, 1, 2, 3, 5, 6, 4, 8, 7, 9):
         work.append((os.path.join(CSRC, "te_inst.cu"), os.path.join(BUILD, f"te_inst_{cb}.o"), [f"-DTE_CB={cb}"]))
     todo = [w for w in work if force or not os.path.exists(w[1]) or os.path.getmtime(w[1]) < newest]
     with cf.ThreadPoolExecutor(max_workers=jobs or min(12, os.cpu_count() or 4)) as ex:

@@ -52,10 +52,10 @@ static int jk_launch(te_pairs* P, double tau, int lane, cudaStream_t st) {
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     // 0: generic thread-per-quartet kernel everywhere; 1: uniform-ket warp kernel for the non-light classes;
-    // 2 (default): split-quartet kernel where instantiated (use_jkq), uniform-ket warp kernel otherwise
+    // 2 (default): split-quartet kernel where instantiated (use_jkq), uniform-ket warp kernel for every other class
     static const int impl = getenv("TE_JK_IMPL") ? atoi(getenv("TE_JK_IMPL")) : 2;
     if constexpr (use_jkq(LA, LB, LC, LD)) {
-        if (impl == 2) {
+        if (impl == 3 || (impl == 2 && jkq_default(LA, LB, LC, LD))) {
             constexpr int QW = 4, QG = jkq_lanes(LA, LB, LC, LD, QW);
             using S = QShape<LA, LB, LC, LD, QG, QW>;
             using Tab = QTab<LA, LB, LC, LD>;
@@ -73,7 +73,7 @@ static int jk_launch(te_pairs* P, double tau, int lane, cudaStream_t st) {
             }
             a.DHb = P->d_DH[TE_CB]; a.DHk = P->d_DH[CK]; a.JHb = P->d_JH[TE_CB]; a.JHk = P->d_JH[CK];
             const int blocks = sms * blocks_per_sm;
-            schedule_w_kernel<<<1, 1024, 0, st>>>(a.qb, a.nb, a.qk, a.nk, a.same, tau, blocks, S::NQ * QW, P->d_tile_start[lane], P->d_task_hi[lane], P->d_ctrl, slot);
+            schedule_w_kernel<<<1, 1024, 0, st>>>(P->d_qmax[TE_CB], a.nb, a.qk, a.nk, a.same, tau, blocks, S::NQ * QW, P->d_tile_start[lane], P->d_task_hi[lane], P->d_ctrl, slot);
             const long long max_tasks = a.nk * ((a.nb + S::NQ * QW - 1) / (S::NQ * QW));
             const unsigned grid = (unsigned)std::min<long long>(max_tasks, (long long)blocks);
             jkq_kernel<LA, LB, LC, LD, QG, QW><<<grid, 32 * QW, S::smem_bytes, st>>>(a, d_tab);
@@ -81,8 +81,8 @@ static int jk_launch(te_pairs* P, double tau, int lane, cudaStream_t st) {
             return TE_OK;
         }
     }
-    if (light || impl == 0) {
-        schedule_kernel<<<1, 1024, 0, st>>>(a.qb, a.nb, a.qk, a.nk, a.same, tau, TB, TK, P->d_tile_start[lane], P->d_ctrl, slot);
+    if ((light && impl < 2) || impl == 0) {
+        schedule_kernel<<<1, 1024, 0, st>>>(P->d_qmax[TE_CB], a.nb, P->d_qmax[CK], a.nk, a.same, tau, TB, TK, P->d_tile_start[lane], P->d_ctrl, slot);
         const long long max_tiles = ((a.nb + TB - 1) / TB) * ((a.nk + TK - 1) / TK);
         const int per_sm = light ? 8 : 16;   // resident CTAs per SM worth of persistent blocks
         const unsigned grid = (unsigned)std::min<long long>(max_tiles, (long long)sms * per_sm);
@@ -98,7 +98,7 @@ static int jk_launch(te_pairs* P, double tau, int lane, cudaStream_t st) {
             if (blocks_per_sm < 1) { set_error("jkw_kernel<%d,%d,%d,%d>: %d bytes of shared memory do not fit", LA, LB, LC, LD, smem); blocks_per_sm = 0; return TE_ERR_CUDA; }
         }
         const int warps = sms * blocks_per_sm;
-        schedule_w_kernel<<<1, 1024, 0, st>>>(a.qb, a.nb, a.qk, a.nk, a.same, tau, warps, S::NL, P->d_tile_start[lane], P->d_task_hi[lane], P->d_ctrl, slot);
+        schedule_w_kernel<<<1, 1024, 0, st>>>(P->d_qmax[TE_CB], a.nb, a.qk, a.nk, a.same, tau, warps, S::NL, P->d_tile_start[lane], P->d_task_hi[lane], P->d_ctrl, slot);
         const long long max_tasks = a.nk * ((a.nb + S::NL - 1) / S::NL);
         const unsigned grid = (unsigned)std::min<long long>(max_tasks, (long long)warps);
         jkw_kernel<LA, LB, LC, LD><<<grid, WARP, smem, st>>>(a);

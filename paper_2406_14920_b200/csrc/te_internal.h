@@ -59,7 +59,8 @@ struct te_pairs {
     double tau_pair = 0.0;
     long long count[TE_NCLASS] = {0};
     te::PairD* d_pair[TE_NCLASS] = {nullptr};
-    double* d_q[TE_NCLASS] = {nullptr};
+    double* d_q[TE_NCLASS] = {nullptr};      // Schwarz bound of every pair
+    double* d_qmax[TE_NCLASS] = {nullptr};   // largest bound of the pair's contracted shell-pair block (non-increasing along the list)
     te::PairIds* d_ids[TE_NCLASS] = {nullptr};
     // Hermite density / Hermite J of every pair (eq. 35), [count][nherm(la+lb)], rebuilt / zeroed by every build
     double* d_DH[TE_NCLASS] = {nullptr};

@@ -16,7 +16,16 @@
 #pragma once
 #include "te_jkw.cuh"
 
+#include <utility>
+
 namespace te {
+
+// compile-time loop: f(std::integral_constant<int, 0>{}), ..., f(std::integral_constant<int, N-1>{}) -- unlike "#pragma unroll"
+// it cannot be declined by the compiler, so every index derived from the counter is a constant
+template <int... Is, class F>
+__device__ __forceinline__ void static_for_impl(std::integer_sequence<int, Is...>, F&& f) { (f(std::integral_constant<int, Is>{}), ...); }
+template <int N, class F>
+__device__ __forceinline__ void static_for(F&& f) { static_for_impl(std::make_integer_sequence<int, N>{}, f); }
 
 // ------------------------------------------------------------------------------------------ class tables
 // All compile-time, evaluated on the host, uploaded once per class and copied to shared memory by every block.
@@ -121,15 +130,15 @@ constexpr int jkq_lanes(int la, int lb, int lc, int ld, int w) {
     return g;
 }
 
-// classes handled by the split-quartet kernel
-// (measured on B200, configs 2 and 3: it wins for every FF ket and for the (PD|DF), (DF|DF) classes; the lighter classes
-// are faster with one quartet per lane)
-constexpr bool use_jkq(int la, int lb, int lc, int ld) {
+// classes for which the split-quartet kernel is instantiated, and those it handles by default (measured on B200, configs 2
+// and 3: it wins for every FF ket and for the (PD|DF), (DF|DF) classes; TE_JK_IMPL=3 forces it wherever it exists)
+constexpr bool use_jkq(int la, int lb, int lc, int ld) { return la + lb + lc + ld >= 3; }
+constexpr bool jkq_default(int la, int lb, int lc, int ld) {
     return (lc + ld == 6) || (lc == 2 && ld == 3 && ((la == 1 && lb == 2) || (la == 2 && lb == 3)));
 }
 
 template <int LA, int LB, int LC, int LD, int G, int W>
-__global__ void __launch_bounds__(32 * W) jkq_kernel(JKArgs a, const QTab<LA, LB, LC, LD>* __restrict__ gtab) {
+__global__ void __launch_bounds__(32 * W, 2) jkq_kernel(JKArgs a, const QTab<LA, LB, LC, LD>* __restrict__ gtab) {
     using S = QShape<LA, LB, LC, LD, G, W>;
     using Tab = QTab<LA, LB, LC, LD>;
     constexpr int LAB = S::LAB, LCD = S::LCD, L = S::L;
@@ -343,12 +352,14 @@ __global__ void __launch_bounds__(32 * W) jkq_kernel(JKArgs a, const QTab<LA, LB
             }
             // ---- exchange part: the ket component pairs (k,l) are dealt over the lanes of the quartet
             if (active && live_k) {
+#pragma unroll 1
                 for (int n = g; n < NKL; n += G) {
                     const int k = tab->kl_k[n], l = tab->kl_l[n];
                     const int q0 = tab->kl_start[n], q1 = tab->kl_start[n + 1];
                     double Yv[NHB];
 #pragma unroll
                     for (int P = 0; P < NHB; ++P) Yv[P] = 0.0;
+#pragma unroll 1
                     for (int q = q0; q < q1; ++q) {
                         const double e = kt[q];
                         const int p = tab->pk[q];
@@ -365,18 +376,19 @@ __global__ void __launch_bounds__(32 * W) jkq_kernel(JKArgs a, const QTab<LA, LB
                                     Yv[tidx<LAB>(t, u, v)] = fma(e, Rrow[v * NQ], Yv[tidx<LAB>(t, u, v)]);
                             }
                     }
-                    // bra Hermite -> Cartesian and K digestion
-                    double kbc[NB], kbd[NB];
+                    // bra Hermite -> Cartesian and K digestion; the larger bra shell (b) is the outer loop so that only the
+                    // 2 * NA accumulators of the smaller one stay live across it
+                    double kac[NA], kad[NA];
 #pragma unroll
-                    for (int jj = 0; jj < NB; ++jj) { kbc[jj] = 0.0; kbd[jj] = 0.0; }
-#pragma unroll
-                    for (int i = 0; i < NA; ++i) {
-                        const int ix = cart_x(LA, i), iy = cart_y(LA, i), iz = cart_z(LA, i);
-                        double kac = 0.0, kad = 0.0;
-                        const double dal = Dad[(i * ND + l) * NQ], dak = Dac[(i * NC + k) * NQ];
-#pragma unroll
-                        for (int jj = 0; jj < NB; ++jj) {
-                            const int jx = cart_x(LB, jj), jy = cart_y(LB, jj), jz = cart_z(LB, jj);
+                    for (int i = 0; i < NA; ++i) { kac[i] = 0.0; kad[i] = 0.0; }
+                    static_for<NB>([&](auto J) {
+                        constexpr int jj = decltype(J)::value;
+                        constexpr int jx = cart_x(LB, jj), jy = cart_y(LB, jj), jz = cart_z(LB, jj);
+                        double kbc = 0.0, kbd = 0.0;
+                        const double dbl = Dbd[(jj * ND + l) * NQ], dbk = Dbc[(jj * NC + k) * NQ];
+                        static_for<NA>([&](auto I) {
+                            constexpr int i = decltype(I)::value;
+                            constexpr int ix = cart_x(LA, i), iy = cart_y(LA, i), iz = cart_z(LA, i);
                             double s = 0.0;
 #pragma unroll
                             for (int t = 0; t <= ix + jx; ++t) {
@@ -392,18 +404,18 @@ __global__ void __launch_bounds__(32 * W) jkq_kernel(JKArgs a, const QTab<LA, LB
                                 s = fma(Eb[((ix * (LB + 1) + jx) * (LAB + 1) + t) * NQ], su, s);
                             }
                             // s = f (ij|kl) without the per-component factors
-                            kac = fma(s, Dbd[(jj * ND + l) * NQ], kac);
-                            kad = fma(s, Dbc[(jj * NC + k) * NQ], kad);
-                            kbc[jj] = fma(s, dal, kbc[jj]);
-                            kbd[jj] = fma(s, dak, kbd[jj]);
-                        }
-                        if (live_kac) atomicAdd(&a.Kt[(ib.offA + i) * nbf + ik.offA + k], kac);
-                        if (live_kad) atomicAdd(&a.Kt[(ib.offA + i) * nbf + ik.offB + l], kad);
-                    }
+                            kac[i] = fma(s, dbl, kac[i]);
+                            kad[i] = fma(s, dbk, kad[i]);
+                            kbc = fma(s, Dad[(i * ND + l) * NQ], kbc);
+                            kbd = fma(s, Dac[(i * NC + k) * NQ], kbd);
+                        });
+                        if (live_kbc) atomicAdd(&a.Kt[(ib.offB + jj) * nbf + ik.offA + k], kbc);
+                        if (live_kbd) atomicAdd(&a.Kt[(ib.offB + jj) * nbf + ik.offB + l], kbd);
+                    });
 #pragma unroll
-                    for (int jj = 0; jj < NB; ++jj) {
-                        if (live_kbc) atomicAdd(&a.Kt[(ib.offB + jj) * nbf + ik.offA + k], kbc[jj]);
-                        if (live_kbd) atomicAdd(&a.Kt[(ib.offB + jj) * nbf + ik.offB + l], kbd[jj]);
+                    for (int i = 0; i < NA; ++i) {
+                        if (live_kac) atomicAdd(&a.Kt[(ib.offA + i) * nbf + ik.offA + k], kac[i]);
+                        if (live_kad) atomicAdd(&a.Kt[(ib.offA + i) * nbf + ik.offB + l], kad[i]);
                     }
                 }
             }

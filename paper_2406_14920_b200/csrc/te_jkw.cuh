@@ -37,7 +37,11 @@ struct WShape {
     static constexpr int NNZK = nnz_e(LC, LD);
     static constexpr int NE1 = (LC + 1) * (LD + 1) * (LCD + 1);
     // K_?c accumulators / D_?c blocks of the smaller ket shell stay in registers for the whole quartet when small
-    static constexpr bool KEEPC = (NA + NB) * NC <= 24;
+    // UNR: the loops over the ket component pairs (k,l) and their Hermite boxes are fully unrolled, so every table offset and
+    // accumulator index is a compile-time constant (no row-table lookups, no dynamically indexed register arrays)
+    static constexpr bool UNR = NHB * NNZK + nnz_e(LA, LB) * NC * ND <= 6000;
+    static constexpr int UNK = UNR ? 128 : 1;
+    static constexpr bool KEEPC = UNR && (NA + NB) * NC <= 24;
     // NL = lanes of the warp that hold a quartet (R column stride).  Measured on B200: narrowing the warp to 8 lanes for L >= 10
     // (4x more resident warps) made (DF|DF) 2.4x SLOWER -- these kernels are bound by per-warp instruction / local-memory
     // throughput, not by latency -- so every lane holds a quartet.
@@ -87,6 +91,8 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
     constexpr int LAB = S::LAB, LCD = S::LCD, L = S::L;
     constexpr int NA = S::NA, NB = S::NB, NC = S::NC, ND = S::ND, NHB = S::NHB;
     constexpr bool KEEPC = S::KEEPC;
+    constexpr bool UNR = S::UNR;
+    constexpr int UNK = S::UNK;
     constexpr int NL = S::NL;
     constexpr unsigned FULLMASK = 0xffffffffu;
     extern __shared__ double sm[];
@@ -174,10 +180,41 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
             }
             if (!__any_sync(FULLMASK, active)) continue;
             const bool any_jcd = __any_sync(FULLMASK, live_jcd);
+            // Runs of lanes whose bras are primitive pairs of ONE contracted shell pair (the lists are shell-pair-major) share every
+            // bra-side output address: their contributions are summed by a segmented shuffle reduction and the run's first lane
+            // issues the atomic.  dist = lanes from this one to the end of its run.
+            const int key = (lane < NL && bi < b_hi) ? (int)(ib.shA * ns + ib.shB) : -1 - lane;
+            const int prev = __shfl_up_sync(FULLMASK, key, 1);
+            const bool head = lane == 0 || key != prev;
+            const unsigned heads = __ballot_sync(FULLMASK, head);
+            const unsigned above = lane == 31 ? 0u : (heads >> (lane + 1)) << (lane + 1);
+            const int dist = (above ? __ffs(above) - 1 : 32) - lane;
+            const int maxdist = __reduce_max_sync(FULLMASK, dist);
+            const bool runs = maxdist > 1;   // warp-uniform: without runs every lane adds its own contribution directly
+            auto flush = [&](bool live, double v, double* addr) {
+                if (runs) {
+                    v = live ? v : 0.0;
+                    for (int o = 1; o < maxdist; o <<= 1) {
+                        const double t = __shfl_down_sync(FULLMASK, v, o);
+                        if (o < dist) v += t;
+                    }
+                    if (head && v != 0.0) atomicAdd(addr, v);
+                } else if (live) {
+                    atomicAdd(addr, v);
+                }
+            };
             double f = 1.0;
             double Ebx[LA + 1][LB + 1][LAB + 1], Eby[LA + 1][LB + 1][LAB + 1], Ebz[LA + 1][LB + 1][LAB + 1];
             double dab[NA * NB], jab[NA * NB];
             double dbc[KEEPC ? NB * NC : 1], dac[KEEPC ? NA * NC : 1], kac[KEEPC ? NA * NC : 1], kbc[KEEPC ? NB * NC : 1];
+#pragma unroll
+            for (int x = 0; x < NA * NB; ++x) jab[x] = 0.0;
+            if (KEEPC) {
+#pragma unroll
+                for (int x = 0; x < NA * NC; ++x) kac[x] = 0.0;
+#pragma unroll
+                for (int x = 0; x < NB * NC; ++x) kbc[x] = 0.0;
+            }
             const double* Da = nullptr; const double* Db = nullptr;   // rows of the scaled density at the bra's AOs
             if (active) {
                 ++nlive;
@@ -204,39 +241,55 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
 #pragma unroll
                 for (int i = 0; i < NA; ++i)
 #pragma unroll
-                    for (int jj = 0; jj < NB; ++jj) { dab[i * NB + jj] = Da[i * nbf + ib.offB + jj]; jab[i * NB + jj] = 0.0; }
+                    for (int jj = 0; jj < NB; ++jj) dab[i * NB + jj] = Da[i * nbf + ib.offB + jj];
                 if (KEEPC) {
 #pragma unroll
                     for (int k = 0; k < NC; ++k) {
 #pragma unroll
-                        for (int i = 0; i < NA; ++i) { dac[i * NC + k] = Da[i * nbf + ik.offA + k]; kac[i * NC + k] = 0.0; }
+                        for (int i = 0; i < NA; ++i) dac[i * NC + k] = Da[i * nbf + ik.offA + k];
 #pragma unroll
-                        for (int jj = 0; jj < NB; ++jj) { dbc[jj * NC + k] = Db[jj * nbf + ik.offA + k]; kbc[jj * NC + k] = 0.0; }
+                        for (int jj = 0; jj < NB; ++jj) dbc[jj * NC + k] = Db[jj * nbf + ik.offA + k];
                     }
                 }
             }
             int ptr = 0;
+#pragma unroll UNK
             for (int l = 0; l < ND; ++l) {
                 const int lx = cart_x(LD, l), ly = cart_y(LD, l), lz = cart_z(LD, l);
                 double dal[NA], dbl[NB], kal[NA], kbl[NB];
+#pragma unroll
+                for (int i = 0; i < NA; ++i) kal[i] = 0.0;
+#pragma unroll
+                for (int jj = 0; jj < NB; ++jj) kbl[jj] = 0.0;
                 if (active) {
 #pragma unroll
-                    for (int i = 0; i < NA; ++i) { dal[i] = Da[i * nbf + ik.offB + l]; kal[i] = 0.0; }
+                    for (int i = 0; i < NA; ++i) dal[i] = Da[i * nbf + ik.offB + l];
 #pragma unroll
-                    for (int jj = 0; jj < NB; ++jj) { dbl[jj] = Db[jj * nbf + ik.offB + l]; kbl[jj] = 0.0; }
+                    for (int jj = 0; jj < NB; ++jj) dbl[jj] = Db[jj * nbf + ik.offB + l];
                 }
+#pragma unroll UNK
                 for (int k = 0; k < NC; ++k) {
                     const int sx = cart_x(LC, k) + lx, sy = cart_y(LC, k) + ly, sz = cart_z(LC, k) + lz;
                     double jkl = 0.0;
+                    double kak[KEEPC ? 1 : NA], kbk[KEEPC ? 1 : NB];
+                    if (!KEEPC) {
+#pragma unroll
+                        for (int i = 0; i < NA; ++i) kak[i] = 0.0;
+#pragma unroll
+                        for (int jj = 0; jj < NB; ++jj) kbk[jj] = 0.0;
+                    }
                     if (active) {
                         // ---- ket Hermite -> Cartesian for this (k,l): Y_P = sum_Q E~_Q R_{P+Q}
                         double Yv[NHB];
 #pragma unroll
                         for (int P = 0; P < NHB; ++P) Yv[P] = 0.0;
                         const double* ktp = kt + ptr;
+#pragma unroll UNK
                         for (int t2 = 0; t2 <= sx; ++t2)
+#pragma unroll UNK
                             for (int u2 = 0; u2 <= sy; ++u2) {
                                 const unsigned short* rt = rowtab + t2 * 13 + u2;
+#pragma unroll UNK
                                 for (int v2 = 0; v2 <= sz; ++v2) {
                                     const double e = *ktp++;
                                     const double* Rq = Rl + v2 * NL;
@@ -244,7 +297,7 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                                     for (int t = 0; t <= LAB; ++t)
 #pragma unroll
                                         for (int u = 0; u <= LAB - t; ++u) {
-                                            const double* Rrow = Rq + (int)rt[t * 13 + u] * NL;
+                                            const double* Rrow = Rq + (UNR ? tidx<L>(t + t2, u + u2, 0) : (int)rt[t * 13 + u]) * NL;
 #pragma unroll
                                             for (int v = 0; v <= LAB - t - u; ++v)
                                                 Yv[tidx<LAB>(t, u, v)] = fma(e, Rrow[v * NL], Yv[tidx<LAB>(t, u, v)]);
@@ -252,12 +305,12 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                                 }
                             }
                         // ---- bra Hermite -> Cartesian and digestion
-                        double dbk[KEEPC ? 1 : NB], dak[KEEPC ? 1 : NA], kak[KEEPC ? 1 : NA], kbk[KEEPC ? 1 : NB];
+                        double dbk[KEEPC ? 1 : NB], dak[KEEPC ? 1 : NA];
                         if (!KEEPC) {
 #pragma unroll
-                            for (int i = 0; i < NA; ++i) { dak[i] = Da[i * nbf + ik.offA + k]; kak[i] = 0.0; }
+                            for (int i = 0; i < NA; ++i) dak[i] = Da[i * nbf + ik.offA + k];
 #pragma unroll
-                            for (int jj = 0; jj < NB; ++jj) { dbk[jj] = Db[jj * nbf + ik.offA + k]; kbk[jj] = 0.0; }
+                            for (int jj = 0; jj < NB; ++jj) dbk[jj] = Db[jj * nbf + ik.offA + k];
                         }
                         const double dkl = dcd[k * ND + l];
 #pragma unroll
@@ -295,17 +348,13 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                                 }
                             }
                         }
-                        if (!KEEPC) {
-                            if (live_kac) {
-#pragma unroll
-                                for (int i = 0; i < NA; ++i) atomicAdd(&a.Kt[(ib.offA + i) * nbf + ik.offA + k], kak[i]);
-                            }
-                            if (live_kbc) {
-#pragma unroll
-                                for (int jj = 0; jj < NB; ++jj) atomicAdd(&a.Kt[(ib.offB + jj) * nbf + ik.offA + k], kbk[jj]);
-                            }
-                        }
                         if (!live_jcd) jkl = 0.0;
+                    }
+                    if (!KEEPC) {
+#pragma unroll
+                        for (int i = 0; i < NA; ++i) flush(live_kac, kak[i], &a.Kt[(ib.offA + i) * nbf + ik.offA + k]);
+#pragma unroll
+                        for (int jj = 0; jj < NB; ++jj) flush(live_kbc, kbk[jj], &a.Kt[(ib.offB + jj) * nbf + ik.offA + k]);
                     }
                     ptr += (sx + 1) * (sy + 1) * (sz + 1);
                     if (any_jcd) {
@@ -314,38 +363,24 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                         if (lane == 0) atomicAdd(&a.Jt[(ik.offA + k) * nbf + ik.offB + l], 2.0 * jkl);
                     }
                 }
-                if (active) {
-                    if (live_kad) {
 #pragma unroll
-                        for (int i = 0; i < NA; ++i) atomicAdd(&a.Kt[(ib.offA + i) * nbf + ik.offB + l], kal[i]);
-                    }
-                    if (live_kbd) {
+                for (int i = 0; i < NA; ++i) flush(live_kad, kal[i], &a.Kt[(ib.offA + i) * nbf + ik.offB + l]);
 #pragma unroll
-                        for (int jj = 0; jj < NB; ++jj) atomicAdd(&a.Kt[(ib.offB + jj) * nbf + ik.offB + l], kbl[jj]);
-                    }
-                }
+                for (int jj = 0; jj < NB; ++jj) flush(live_kbd, kbl[jj], &a.Kt[(ib.offB + jj) * nbf + ik.offB + l]);
             }
-            if (active) {
-                if (live_jab) {
 #pragma unroll
-                    for (int i = 0; i < NA; ++i)
+            for (int i = 0; i < NA; ++i)
 #pragma unroll
-                        for (int jj = 0; jj < NB; ++jj) atomicAdd(&a.Jt[(ib.offA + i) * nbf + ib.offB + jj], 2.0 * jab[i * NB + jj]);
-                }
-                if (KEEPC) {
-                    if (live_kac) {
+                for (int jj = 0; jj < NB; ++jj) flush(live_jab, 2.0 * jab[i * NB + jj], &a.Jt[(ib.offA + i) * nbf + ib.offB + jj]);
+            if (KEEPC) {
 #pragma unroll
-                        for (int i = 0; i < NA; ++i)
+                for (int i = 0; i < NA; ++i)
 #pragma unroll
-                            for (int k = 0; k < NC; ++k) atomicAdd(&a.Kt[(ib.offA + i) * nbf + ik.offA + k], kac[i * NC + k]);
-                    }
-                    if (live_kbc) {
+                    for (int k = 0; k < NC; ++k) flush(live_kac, kac[i * NC + k], &a.Kt[(ib.offA + i) * nbf + ik.offA + k]);
 #pragma unroll
-                        for (int jj = 0; jj < NB; ++jj)
+                for (int jj = 0; jj < NB; ++jj)
 #pragma unroll
-                            for (int k = 0; k < NC; ++k) atomicAdd(&a.Kt[(ib.offB + jj) * nbf + ik.offA + k], kbc[jj * NC + k]);
-                    }
-                }
+                    for (int k = 0; k < NC; ++k) flush(live_kbc, kbc[jj * NC + k], &a.Kt[(ib.offB + jj) * nbf + ik.offA + k]);
             }
             __syncwarp();
         }

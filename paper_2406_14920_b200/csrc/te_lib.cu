@@ -186,6 +186,29 @@ __global__ void count_kept_kernel(const double* __restrict__ q_sorted, long long
     if ((threadIdx.x & 31) == 0 && c) atomicAdd(out, c);
 }
 
+// Shell-pair-major order: primitive pairs of one contracted shell pair (A,B) share every J/K output address, so the J/K kernels
+// reduce over runs of them before touching memory.  key = A * nshells + B; bmax[key] = max bound of the block.
+__global__ void block_key_kernel(const PairIds* __restrict__ ids, const double* __restrict__ q, long long n, int nshells,
+                                 unsigned int* __restrict__ key, unsigned int* __restrict__ perm, unsigned long long* __restrict__ bmax) {
+    const long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (x >= n) return;
+    const unsigned int k = (unsigned int)ids[x].shA * (unsigned int)nshells + (unsigned int)ids[x].shB;
+    key[x] = k; perm[x] = (unsigned int)x;
+    atomicMax(&bmax[k], (unsigned long long)__double_as_longlong(q[x]));   // bounds are >= 0: the bit pattern orders like the value
+}
+__global__ void block_max_gather_kernel(const unsigned int* __restrict__ key, long long n, const unsigned long long* __restrict__ bmax,
+                                        double* __restrict__ bm) {
+    const long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (x < n) bm[x] = __longlong_as_double((long long)bmax[key[x]]);
+}
+__global__ void permute_pairs_kernel(const unsigned int* __restrict__ perm, long long n, const PairD* __restrict__ pin, const PairIds* __restrict__ iin,
+                                     const double* __restrict__ qin, PairD* __restrict__ pout, PairIds* __restrict__ iout, double* __restrict__ qout) {
+    const long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (x >= n) return;
+    const unsigned int y = perm[x];
+    pout[x] = pin[y]; iout[x] = iin[y]; qout[x] = qin[y];
+}
+
 extern "C" int te_shellpair_build(const te_basis* b, double tau_pair, te_pairs** out) {
     if (!out) { set_error("te_shellpair_build: out is NULL"); return TE_ERR_BAD_ARG; }
     *out = nullptr;
@@ -233,11 +256,41 @@ extern "C" int te_shellpair_build(const te_basis* b, double tau_pair, te_pairs**
                     cleanup(); set_error("te_shellpair_build: pair allocation failed"); return fail(TE_ERR_ALLOC);
                 }
                 const size_t nh = (size_t)nk * nherm(la + lb) * sizeof(double);
-                if (cudaMalloc(&P->d_DH[cls], nh) != cudaSuccess || cudaMalloc(&P->d_JH[cls], nh) != cudaSuccess) {
+                if (cudaMalloc(&P->d_DH[cls], nh) != cudaSuccess || cudaMalloc(&P->d_JH[cls], nh) != cudaSuccess ||
+                    cudaMalloc(&P->d_qmax[cls], nk * sizeof(double)) != cudaSuccess) {
                     cleanup(); set_error("te_shellpair_build: Hermite buffer allocation failed"); return fail(TE_ERR_ALLOC);
                 }
-                cudaMemcpy(P->d_q[cls], d_qs, nk * sizeof(double), cudaMemcpyDeviceToDevice);
-                if ((rc = launch_pair_fill(la, lb, b, (long long)nk, d_idxs, P->d_pair[cls], P->d_ids[cls])) != TE_OK) { cleanup(); return fail(rc); }
+                // pass 2: pair data of the survivors in bound order, then the shell-pair-major permutation:
+                // stable sort by shell pair, then stable sort by the block's largest bound (descending); inside a block
+                // the pairs stay in bound order
+                PairD* t_pair = nullptr; PairIds* t_ids = nullptr;
+                unsigned int *k0 = nullptr, *k1 = nullptr, *p0 = nullptr, *p1 = nullptr, *p2 = nullptr;
+                unsigned long long* bmax = nullptr; double *bm = nullptr; void* tmp2 = nullptr;
+                const size_t ns2 = (size_t)b->nshells * b->nshells;
+                auto cleanup2 = [&]() { cudaFree(t_pair); cudaFree(t_ids); cudaFree(k0); cudaFree(k1); cudaFree(p0); cudaFree(p1); cudaFree(p2);
+                                        cudaFree(bmax); cudaFree(bm); cudaFree(tmp2); };
+                if (cudaMalloc(&t_pair, nk * sizeof(PairD)) != cudaSuccess || cudaMalloc(&t_ids, nk * sizeof(PairIds)) != cudaSuccess ||
+                    cudaMalloc(&k0, nk * 4) != cudaSuccess || cudaMalloc(&k1, nk * 4) != cudaSuccess || cudaMalloc(&p0, nk * 4) != cudaSuccess ||
+                    cudaMalloc(&p1, nk * 4) != cudaSuccess || cudaMalloc(&p2, nk * 4) != cudaSuccess || cudaMalloc(&bmax, ns2 * 8) != cudaSuccess ||
+                    cudaMalloc(&bm, nk * sizeof(double)) != cudaSuccess) {
+                    cleanup2(); cleanup(); set_error("te_shellpair_build: ordering scratch allocation failed"); return fail(TE_ERR_ALLOC);
+                }
+                if ((rc = launch_pair_fill(la, lb, b, (long long)nk, d_idxs, t_pair, t_ids)) != TE_OK) { cleanup2(); cleanup(); return fail(rc); }
+                cudaMemset(bmax, 0, ns2 * 8);
+                const unsigned gr = (unsigned)((nk + 255) / 256);
+                block_key_kernel<<<gr, 256>>>(t_ids, d_qs, (long long)nk, b->nshells, k0, p0, bmax);
+                size_t tb1 = 0, tb2 = 0;
+                cub::DeviceRadixSort::SortPairs(nullptr, tb1, k0, k1, p0, p1, (int)nk);
+                cub::DeviceRadixSort::SortPairsDescending(nullptr, tb2, bm, d_q, p1, p2, (int)nk);
+                if (cudaMalloc(&tmp2, std::max(tb1, tb2)) != cudaSuccess) { cleanup2(); cleanup(); set_error("cub temp alloc failed"); return fail(TE_ERR_ALLOC); }
+                tb1 = tb2 = std::max(tb1, tb2);
+                cub::DeviceRadixSort::SortPairs(tmp2, tb1, k0, k1, p0, p1, (int)nk);
+                block_max_gather_kernel<<<gr, 256>>>(k1, (long long)nk, bmax, bm);
+                cub::DeviceRadixSort::SortPairsDescending(tmp2, tb2, bm, P->d_qmax[cls], p1, p2, (int)nk);
+                permute_pairs_kernel<<<gr, 256>>>(p2, (long long)nk, t_pair, t_ids, d_qs, P->d_pair[cls], P->d_ids[cls], P->d_q[cls]);
+                cudaError_t e2 = cudaDeviceSynchronize();
+                cleanup2();
+                if (e2 != cudaSuccess) { cleanup(); set_error("te_shellpair_build: %s", cudaGetErrorString(e2)); return fail(TE_ERR_CUDA); }
             }
             cudaError_t e = cudaDeviceSynchronize();
             cleanup();
@@ -272,7 +325,7 @@ extern "C" int te_shellpair_build(const te_basis* b, double tau_pair, te_pairs**
 
 extern "C" void te_pairs_destroy(te_pairs* P) {
     if (!P) return;
-    for (int c = 0; c < TE_NCLASS; ++c) { cudaFree(P->d_pair[c]); cudaFree(P->d_q[c]); cudaFree(P->d_ids[c]); cudaFree(P->d_DH[c]); cudaFree(P->d_JH[c]); }
+    for (int c = 0; c < TE_NCLASS; ++c) { cudaFree(P->d_pair[c]); cudaFree(P->d_q[c]); cudaFree(P->d_ids[c]); cudaFree(P->d_DH[c]); cudaFree(P->d_JH[c]); cudaFree(P->d_qmax[c]); }
     cudaFree(P->d_Ds); cudaFree(P->d_Jt); cudaFree(P->d_Kt); cudaFree(P->d_Dm); cudaFree(P->d_ctrl);
     for (int s = 0; s < te_pairs::NSTREAM; ++s) {
         cudaFree(P->d_tile_start[s]); cudaFree(P->d_task_hi[s]);
@@ -293,20 +346,35 @@ extern "C" int te_pairs_info(const te_pairs* P, long long class_count[TE_NCLASS]
     return TE_OK;
 }
 
+// The lists live on the device in shell-pair-major order (see te_shellpair_build); the exports present them in the order the
+// header promises: Schwarz bound descending (stable, so equal bounds keep their internal order).
+static int bound_order(const te_pairs* P, int cls, std::vector<double>& q, std::vector<long long>& order) {
+    const long long n = P->count[cls];
+    q.resize(n); order.resize(n);
+    TE_CUDA(cudaMemcpy(q.data(), P->d_q[cls], n * sizeof(double), cudaMemcpyDeviceToHost));
+    for (long long i = 0; i < n; ++i) order[i] = i;
+    std::stable_sort(order.begin(), order.end(), [&](long long x, long long y) { return q[x] > q[y]; });
+    return TE_OK;
+}
+
 extern "C" int te_pairs_export(const te_pairs* P, int cls, int* shellA, int* shellB, int* primA, int* primB, double* bound) {
     if (!P || cls < 0 || cls >= TE_NCLASS) { set_error("te_pairs_export: bad handle or class"); return TE_ERR_BAD_ARG; }
     const long long n = P->count[cls];
     if (n == 0) return TE_OK;
     std::vector<PairIds> ids(n);
     TE_CUDA(cudaMemcpy(ids.data(), P->d_ids[cls], n * sizeof(PairIds), cudaMemcpyDeviceToHost));
+    std::vector<double> q; std::vector<long long> order;
+    int rc = bound_order(P, cls, q, order);
+    if (rc != TE_OK) return rc;
     const te_basis* b = P->basis;
     for (long long i = 0; i < n; ++i) {
-        if (shellA) shellA[i] = ids[i].shA;
-        if (shellB) shellB[i] = ids[i].shB;
-        if (primA) primA[i] = b->prim_iprim[ids[i].m];
-        if (primB) primB[i] = b->prim_iprim[ids[i].n];
+        const PairIds& id = ids[order[i]];
+        if (shellA) shellA[i] = id.shA;
+        if (shellB) shellB[i] = id.shB;
+        if (primA) primA[i] = b->prim_iprim[id.m];
+        if (primB) primB[i] = b->prim_iprim[id.n];
+        if (bound) bound[i] = q[order[i]];
     }
-    if (bound) TE_CUDA(cudaMemcpy(bound, P->d_q[cls], n * sizeof(double), cudaMemcpyDeviceToHost));
     return TE_OK;
 }
 
@@ -316,10 +384,14 @@ extern "C" int te_pairs_export_geom(const te_pairs* P, int cls, double* P_xyz, d
     if (n == 0) return TE_OK;
     std::vector<PairD> pd(n);
     TE_CUDA(cudaMemcpy(pd.data(), P->d_pair[cls], n * sizeof(PairD), cudaMemcpyDeviceToHost));
+    std::vector<double> q; std::vector<long long> order;
+    int rc = bound_order(P, cls, q, order);
+    if (rc != TE_OK) return rc;
     for (long long i = 0; i < n; ++i) {
-        if (P_xyz) for (int d = 0; d < 3; ++d) P_xyz[3 * i + d] = pd[i].P[d];
-        if (p_exp) p_exp[i] = pd[i].p;
-        if (prefactor) prefactor[i] = pd[i].pref;
+        const PairD& x = pd[order[i]];
+        if (P_xyz) for (int d = 0; d < 3; ++d) P_xyz[3 * i + d] = x.P[d];
+        if (p_exp) p_exp[i] = x.p;
+        if (prefactor) prefactor[i] = x.pref;
     }
     return TE_OK;
 }
