@@ -26,6 +26,9 @@ import numpy as np  # noqa: E402
 
 METRIC = "primitive_shell_quartets_per_s"
 UNIT = "quartets/s"
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the class kernels captured with ncu --set full
+# (profiles/r1_ncu_full_final_cfg2.txt); other kernels / configs have no capture and report null
+NCU_DRAM_BYTES = {(2, "(PD|PF)"): 3.97e6, (2, "(SP|DF)"): 5.39e6, (2, "(PF|DF)"): 2.81e6}
 CONFIG_NAMES = {1: "cfg1_tiny", 2: "cfg2_small_organic", 3: "cfg3_water16", 4: "cfg4_metal_complex",
                 5: "cfg5_large_organic"}
 
@@ -202,7 +205,9 @@ def main_ours(args, rank, world):
     q, _ = pairs.stats()
     live = int(q.sum())
     npairs_nonempty = sum(1 for cb in range(10) for ck in range(cb, 10) if pairs.class_count[cb] and pairs.class_count[ck])
-    launches_per_step = 3 + 2 * npairs_nonempty               # scale, bounds, finish + (schedule, jk) per class pair
+    nclasses_nonempty = sum(1 for c in range(10) if pairs.class_count[c])
+    # scale, bounds, finish + (Hermite density, Hermite J) per pair class + (schedule, J/K kernel) per class pair
+    launches_per_step = 3 + 2 * nclasses_nonempty + 2 * npairs_nonempty
 
     # end to end through the host entry point: pinned host D in, pinned host J/K out, copies inside the timed region
     Dh = torch.tensor(prob.D).pin_memory()
@@ -247,8 +252,9 @@ def main_ours(args, rank, world):
         "jk_build_s_per_iter": step_s, "pair_build_s": t_setup,
         "model_flops_per_build": total_flops, "fp64_tflops_algorithmic": total_flops / step_s / 1e12,
         "fp64_frac_of_peak": total_flops / step_s / 1e12 / peak,
-        "roofline": {"bound": "alu", "kernel": f"jk_kernel ({te.CLASS_NAMES[cb]}|{te.CLASS_NAMES[ck]})",
-                     "achieved": dom_ach, "peak": peak, "unit": "TFLOP/s", "frac": dom_ach / peak, "traffic": None,
+        "roofline": {"bound": "alu", "kernel": f"J/K class kernel ({te.CLASS_NAMES[cb]}|{te.CLASS_NAMES[ck]})",
+                     "achieved": dom_ach, "peak": peak, "unit": "TFLOP/s", "frac": dom_ach / peak,
+                     "traffic": NCU_DRAM_BYTES.get((args.config, f"({te.CLASS_NAMES[cb]}|{te.CLASS_NAMES[ck]})")),
                      "peak_source": "te_measure_fp64_peak: register-resident DFMA chains measured in this run "
                                     "(MEASURED_PEAKS.json has no FP64 entry; nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2)",
                      "top_kernels_ms": per_class},
