@@ -16,16 +16,7 @@
 #pragma once
 #include "te_jkw.cuh"
 
-#include <utility>
-
 namespace te {
-
-// compile-time loop: f(std::integral_constant<int, 0>{}), ..., f(std::integral_constant<int, N-1>{}) -- unlike "#pragma unroll"
-// it cannot be declined by the compiler, so every index derived from the counter is a constant
-template <int... Is, class F>
-__device__ __forceinline__ void static_for_impl(std::integer_sequence<int, Is...>, F&& f) { (f(std::integral_constant<int, Is>{}), ...); }
-template <int N, class F>
-__device__ __forceinline__ void static_for(F&& f) { static_for_impl(std::make_integer_sequence<int, N>{}, f); }
 
 // ------------------------------------------------------------------------------------------ class tables
 // All compile-time, evaluated on the host, uploaded once per class and copied to shared memory by every block.
@@ -139,7 +130,7 @@ constexpr bool jkq_default(int la, int lb, int lc, int ld) {
 }
 
 template <int LA, int LB, int LC, int LD, int G, int W>
-__global__ void __launch_bounds__(32 * W, 2) jkq_kernel(JKArgs a, const QTab<LA, LB, LC, LD>* __restrict__ gtab) {
+__global__ void __launch_bounds__(32 * W, (nherm(LA + LB) <= 10 ? 4 : 2)) jkq_kernel(JKArgs a, const QTab<LA, LB, LC, LD>* __restrict__ gtab) {
     using S = QShape<LA, LB, LC, LD, G, W>;
     using Tab = QTab<LA, LB, LC, LD>;
     constexpr int LAB = S::LAB, LCD = S::LCD, L = S::L;

@@ -9,7 +9,16 @@
 #pragma once
 #include "te_kernels.cuh"
 
+#include <utility>
+
 namespace te {
+
+// compile-time loop: f(std::integral_constant<int, 0>{}), ..., f(std::integral_constant<int, N-1>{}) -- unlike "#pragma unroll"
+// it cannot be declined by the compiler, so every index derived from the counter is a constant
+template <int... Is, class F>
+__device__ __forceinline__ void static_for_impl(std::integer_sequence<int, Is...>, F&& f) { (f(std::integral_constant<int, Is>{}), ...); }
+template <int N, class F>
+__device__ __forceinline__ void static_for(F&& f) { static_for_impl(std::make_integer_sequence<int, N>{}, f); }
 
 // ROW[L][t][u] = index of (t,u,0) in the nested tetrahedral layout tidx<L>; (t,u,v) sits v entries further.
 struct RowTab {
@@ -102,7 +111,6 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
     double* const dcd = e1 + 3 * S::NE1;
     const int lane = threadIdx.x;
     double* const Rl = Rsm + (lane < NL ? lane : 0);   // lanes >= NL never hold a quartet
-    const unsigned short* const rowtab = c_rowtab.v + L * 169;
 
     const unsigned long long ntasks = a.ctrl->ntiles[a.slot];
     const long long span = (long long)NL * a.ctrl->chunk[a.slot];
@@ -284,26 +292,48 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
 #pragma unroll
                         for (int P = 0; P < NHB; ++P) Yv[P] = 0.0;
                         const double* ktp = kt + ptr;
-#pragma unroll UNK
-                        for (int t2 = 0; t2 <= sx; ++t2)
-#pragma unroll UNK
-                            for (int u2 = 0; u2 <= sy; ++u2) {
-                                const unsigned short* rt = rowtab + t2 * 13 + u2;
-#pragma unroll UNK
-                                for (int v2 = 0; v2 <= sz; ++v2) {
-                                    const double e = *ktp++;
-                                    const double* Rq = Rl + v2 * NL;
+                        if constexpr (UNR) {
 #pragma unroll
-                                    for (int t = 0; t <= LAB; ++t)
+                            for (int t2 = 0; t2 <= sx; ++t2)
 #pragma unroll
-                                        for (int u = 0; u <= LAB - t; ++u) {
-                                            const double* Rrow = Rq + (UNR ? tidx<L>(t + t2, u + u2, 0) : (int)rt[t * 13 + u]) * NL;
+                                for (int u2 = 0; u2 <= sy; ++u2)
 #pragma unroll
-                                            for (int v = 0; v <= LAB - t - u; ++v)
-                                                Yv[tidx<LAB>(t, u, v)] = fma(e, Rrow[v * NL], Yv[tidx<LAB>(t, u, v)]);
+                                    for (int v2 = 0; v2 <= sz; ++v2) {
+                                        const double e = *ktp++;
+#pragma unroll
+                                        for (int t = 0; t <= LAB; ++t)
+#pragma unroll
+                                            for (int u = 0; u <= LAB - t; ++u)
+#pragma unroll
+                                                for (int v = 0; v <= LAB - t - u; ++v)
+                                                    Yv[tidx<LAB>(t, u, v)] = fma(e, Rl[(tidx<L>(t + t2, u + u2, 0) + v + v2) * NL], Yv[tidx<LAB>(t, u, v)]);
+                                    }
+                        } else {
+                            // (t2,u2) run over the whole ket triangle at compile time and the (warp-uniform) box limits of this
+                            // (k,l) skip the rest, so every R offset is an immediate: one running pointer per v2, no row table
+                            static_for<LCD + 1>([&](auto T2) {
+                                constexpr int t2 = decltype(T2)::value;
+                                if (t2 <= sx) {
+                                    static_for<LCD + 1 - t2>([&](auto U2) {
+                                        constexpr int u2 = decltype(U2)::value;
+                                        if (u2 <= sy) {
+                                            const double* Rq = Rl;
+#pragma unroll 1
+                                            for (int v2 = 0; v2 <= sz; ++v2, Rq += NL) {
+                                                const double e = *ktp++;
+#pragma unroll
+                                                for (int t = 0; t <= LAB; ++t)
+#pragma unroll
+                                                    for (int u = 0; u <= LAB - t; ++u)
+#pragma unroll
+                                                        for (int v = 0; v <= LAB - t - u; ++v)
+                                                            Yv[tidx<LAB>(t, u, v)] = fma(e, Rq[(tidx<L>(t + t2, u + u2, 0) + v) * NL], Yv[tidx<LAB>(t, u, v)]);
+                                            }
                                         }
+                                    });
                                 }
-                            }
+                            });
+                        }
                         // ---- bra Hermite -> Cartesian and digestion
                         double dbk[KEEPC ? 1 : NB], dak[KEEPC ? 1 : NA];
                         if (!KEEPC) {
