@@ -25,17 +25,18 @@ struct QTab {
     static constexpr int LAB = LA + LB, LCD = LC + LD, L = LAB + LCD;
     static constexpr int NC = ncart(LC), ND = ncart(LD), NKL = NC * ND, NNZK = nnz_e(LC, LD);
     static constexpr int NHB = nherm(LAB), NHK = nherm(LCD), NR = nherm(L);
+    // R recurrence recipe, elements ordered by degree n = t+u+v: R[e] = XYZ[dir] * R[s1] + c2 * R[s2]   (eq. 22-24);
+    // rc[r] = {e, s1, s2, dir | c2 << 2}, read with one 8-byte load (first member: 8-byte aligned)
+    unsigned short rc[NR][4];
     // ket component pairs in processing order (largest Hermite box first, so the lanes of a round do similar work)
     unsigned short kl_k[NKL], kl_l[NKL], kl_start[NKL + 1];
     unsigned short pk[NNZK];       // box entry -> t2 | u2 << 4 | v2 << 8
     unsigned short qkl[NNZK];      // box entry -> position of its (k,l) in the processing order
     unsigned short rowtab[13 * 13];   // (T,U) -> index of R_{T,U,0} in the tetrahedral layout of order L
     unsigned short hb[NHB], hk[NHK];  // Hermite index -> t | u << 4 | v << 8 (bra / ket tetrahedra)
-    // R recurrence recipe, elements ordered by degree n = t+u+v: R[e] = XYZ[dir] * R[s1] + c2 * R[s2]   (eq. 22-24)
-    unsigned short rc_e[NR], rc_s1[NR], rc_s2[NR], rc_dc[NR];   // rc_dc = dir | c2 << 2
     unsigned short deg_start[14];
 
-    constexpr QTab() : kl_k{}, kl_l{}, kl_start{}, pk{}, qkl{}, rowtab{}, hb{}, hk{}, rc_e{}, rc_s1{}, rc_s2{}, rc_dc{}, deg_start{} {
+    constexpr QTab() : rc{}, kl_k{}, kl_l{}, kl_start{}, pk{}, qkl{}, rowtab{}, hb{}, hk{}, deg_start{} {
         int order[NKL] = {}, size[NKL] = {};
         for (int k = 0; k < NC; ++k)
             for (int l = 0; l < ND; ++l) {
@@ -82,8 +83,8 @@ struct QTab {
                         else if (u > 0) { dir = 1; s1 = tidx<L>(t, u - 1, v); if (u > 1) { s2 = tidx<L>(t, u - 2, v); c2 = u - 1; } }
                         else { dir = 2; s1 = tidx<L>(t, u, v - 1); if (v > 1) { s2 = tidx<L>(t, u, v - 2); c2 = v - 1; } }
                     }
-                    rc_e[r] = (unsigned short)tidx<L>(t, u, v); rc_s1[r] = (unsigned short)s1; rc_s2[r] = (unsigned short)s2;
-                    rc_dc[r] = (unsigned short)(dir | (c2 << 2));
+                    rc[r][0] = (unsigned short)tidx<L>(t, u, v); rc[r][1] = (unsigned short)s1; rc[r][2] = (unsigned short)s2;
+                    rc[r][3] = (unsigned short)(dir | (c2 << 2));
                     ++r;
                 }
         }
@@ -106,7 +107,7 @@ struct QShape {
 };
 
 // lanes per quartet: enough ket component pairs per lane to keep the lanes busy, few enough quartets per warp that a block's
-// shared memory stays under ~72 KB (three blocks per SM)
+// shared memory fits the number of blocks per SM the registers allow
 constexpr int jkq_smem(int la, int lb, int lc, int ld, int g, int w) {
     const int lab = la + lb, lcd = lc + ld, L = lab + lcd;
     const int ndb = ncart(lb) * ncart(ld) + ncart(lb) * ncart(lc) + ncart(la) * ncart(ld) + ncart(la) * ncart(lc);
@@ -117,7 +118,9 @@ constexpr int jkq_smem(int la, int lb, int lc, int ld, int g, int w) {
 constexpr int jkq_lanes(int la, int lb, int lc, int ld, int w) {
     const int nkl = ncart(lc) * ncart(ld);
     int g = nkl >= 100 ? 16 : nkl >= 30 ? 8 : nkl >= 10 ? 4 : 2;
-    while (g < 32 && jkq_smem(la, lb, lc, ld, g, w) > 72 * 1024) g *= 2;
+    // blocks per SM are set by registers (launch bounds: 4 for light bras, 2 otherwise); shared memory may use the rest
+    const int cap = nherm(la + lb) <= 10 ? 54 * 1024 : 110 * 1024;
+    while (g < 32 && jkq_smem(la, lb, lc, ld, g, w) > cap) g *= 2;
     return g;
 }
 
@@ -297,7 +300,8 @@ __global__ void __launch_bounds__(32 * W, (nherm(LA + LB) <= 10 ? 4 : 2)) jkq_ke
                         const int s0 = tab->deg_start[n], cnt = tab->deg_start[n + 1] - s0;
                         if (active) {
                             for (int x = g; x < cnt; x += G) {
-                                const int e = tab->rc_e[s0 + x], s1 = tab->rc_s1[s0 + x], s2 = tab->rc_s2[s0 + x], dc = tab->rc_dc[s0 + x];
+                                const uint2 rc = *reinterpret_cast<const uint2*>(&tab->rc[s0 + x][0]);
+                                const int e = rc.x & 0xffff, s1 = rc.x >> 16, s2 = rc.y & 0xffff, dc = rc.y >> 16;
                                 const int dir = dc & 3;
                                 const double c = dir == 0 ? X : (dir == 1 ? Y_ : Z);
                                 Rs[e * NQ] = fma((double)(dc >> 2), Rs[s2 * NQ], c * Rs[s1 * NQ]);
@@ -315,12 +319,16 @@ __global__ void __launch_bounds__(32 * W, (nherm(LA + LB) <= 10 ? 4 : 2)) jkq_ke
                     const int p = tab->hb[P];
                     const int t = p & 15, u = (p >> 4) & 15, v = p >> 8;
                     double s = 0.0;
-                    int Q = 0;
-                    for (int t2 = 0; t2 <= LCD; ++t2)
-                        for (int u2 = 0; u2 <= LCD - t2; ++u2) {
-                            const double* Rrow = Rs + ((int)rt[(t + t2) * 13 + u + u2] + v) * NQ;
-                            for (int v2 = 0; v2 <= LCD - t2 - u2; ++v2, ++Q) s = fma(sdhk[Q], Rrow[v2 * NQ], s);
-                        }
+                    const unsigned short* rtp = rt + t * 13 + u;
+                    static_for<LCD + 1>([&](auto T2) {
+                        constexpr int t2 = decltype(T2)::value;
+                        static_for<LCD + 1 - t2>([&](auto U2) {
+                            constexpr int u2 = decltype(U2)::value;
+                            const double* Rrow = Rs + ((int)rtp[t2 * 13 + u2] + v) * NQ;
+#pragma unroll
+                            for (int v2 = 0; v2 <= LCD - t2 - u2; ++v2) s = fma(sdhk[tidx<LCD>(t2, u2, v2)], Rrow[v2 * NQ], s);
+                        });
+                    });
                     atomicAdd(&a.JHb[bi * NHB + P], 2.0 * s);
                 }
             }
@@ -332,12 +340,16 @@ __global__ void __launch_bounds__(32 * W, (nherm(LA + LB) <= 10 ? 4 : 2)) jkq_ke
                         const int p = tab->hk[Q];
                         const int t2 = p & 15, u2 = (p >> 4) & 15, v2 = p >> 8;
                         double s = 0.0;
-                        int P = 0;
-                        for (int t = 0; t <= LAB; ++t)
-                            for (int u = 0; u <= LAB - t; ++u) {
-                                const double* Rrow = Rs + ((int)rt[(t + t2) * 13 + u + u2] + v2) * NQ;
-                                for (int v = 0; v <= LAB - t - u; ++v, ++P) s = fma(dhb[P * NQ], Rrow[v * NQ], s);
-                            }
+                        const unsigned short* rtp = rt + t2 * 13 + u2;
+                        static_for<LAB + 1>([&](auto T) {
+                            constexpr int t = decltype(T)::value;
+                            static_for<LAB + 1 - t>([&](auto U) {
+                                constexpr int u = decltype(U)::value;
+                                const double* Rrow = Rs + ((int)rtp[t * 13 + u] + v2) * NQ;
+#pragma unroll
+                                for (int v = 0; v <= LAB - t - u; ++v) s = fma(dhb[tidx<LAB>(t, u, v) * NQ], Rrow[v * NQ], s);
+                            });
+                        });
                         jhk[x] += s;
                     }
                 }
