@@ -124,12 +124,14 @@ constexpr int jkq_lanes(int la, int lb, int lc, int ld, int w) {
     return g;
 }
 
-// classes for which the split-quartet kernel is instantiated, and those it handles by default.  Measured on B200 (configs 2
-// and 3, per-class CUDA-event times): it wins for every FF ket, for d/f-heavy bras (la+lb >= 4) against kets with lc+ld >= 4
-// and for (PD|DD), (PD|DF); one quartet per lane (uniform-ket kernel) wins elsewhere.  TE_JK_IMPL=3 forces it wherever it exists.
+// classes for which the split-quartet kernel is instantiated, and those it handles by default.  Measured on B200 (configs 2,
+// 3 and 5, per-class CUDA-event times): it wins for every FF ket, for DF kets against bras with la+lb >= 2, for d/f-heavy bras
+// (la+lb >= 4) against kets with lc+ld >= 4, and for (SD|DD), (PD|PF), (PD|DD); one quartet per lane (uniform-ket kernel) wins
+// elsewhere.  TE_JK_IMPL=3 forces it wherever it exists.
 constexpr bool use_jkq(int la, int lb, int lc, int ld) { return la + lb + lc + ld >= 3; }
 constexpr bool jkq_default(int la, int lb, int lc, int ld) {
-    return (lc + ld == 6) || (la + lb >= 4 && lc + ld >= 4) || (la == 1 && lb == 2 && lc == 2);
+    return (lc + ld == 6) || (lc == 2 && ld == 3 && la + lb >= 2) || (la + lb >= 4 && lc + ld >= 4) ||
+           (la == 1 && lb == 2 && lc + ld >= 4) || (la == 0 && lb == 2 && lc == 2 && ld == 2);
 }
 
 template <int LA, int LB, int LC, int LD, int G, int W>

@@ -265,3 +265,41 @@ def test_translation_invariance_on_device(te, torch_):
     moved = Problem(**{**prob.__dict__, "xyz": prob.xyz + np.array([11.0, -7.5, 3.25])})
     _, _, Jm, Km = _gpu_jk(te, torch_, moved)
     assert np.max(np.abs(J - Jm)) < 1e-10 and np.max(np.abs(K - Km)) < 1e-10
+
+
+# ------------------------------------------------------------------------- every kernel family, every class
+_IMPL_CHILD = r"""
+import sys, numpy as np, torch
+sys.path.insert(0, {root!r})
+import paper_2406_14920_b200 as te
+import oracle
+from synth import make_config, subset_atoms
+worst = 0.0
+for prob in (make_config(1), subset_atoms(make_config(2), [0, 1, 12, 13])):   # all 55 classes unscreened; contracted s/p runs, screened
+    b = te.Basis.from_problem(prob)
+    pr = b.shellpair_build(prob.tau_pair)
+    J, K = pr.build_jk(torch.tensor(prob.D, device="cuda"), threshold=prob.tau_jk)
+    torch.cuda.synchronize()
+    o = oracle.Oracle(prob)
+    o.build_pairs(prob.tau_pair)
+    Jo, Ko, st = o.jk_o2(prob.D, prob.tau_jk)
+    q, _ = pr.stats()
+    assert abs(int(q.sum()) - st["live_quartets"]) <= max(10, st["borderline"]), (int(q.sum()), st)
+    worst = max(worst, float(np.max(np.abs(J.cpu().numpy() - Jo))), float(np.max(np.abs(K.cpu().numpy() - Ko))))
+print("WORST", worst)
+"""
+
+
+@pytest.mark.parametrize("impl", ["0", "1", "3"])
+def test_jk_every_kernel_family(te, impl):
+    """TE_JK_IMPL selects the kernel family per class at library load (0: generic thread-per-quartet kernel, 1: uniform-ket
+    warp kernel + generic light classes, 3: split-quartet kernel wherever it is instantiated; the default policy is what every
+    other test runs).  Each family must meet the same bar on all 55 classes."""
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, TE_JK_IMPL=impl)
+    r = subprocess.run([sys.executable, "-c", _IMPL_CHILD.format(root=root)], env=env, capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
+    worst = float(r.stdout.strip().splitlines()[-1].split()[1])
+    assert worst <= TOL_JK, worst
