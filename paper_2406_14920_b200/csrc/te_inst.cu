@@ -1,6 +1,7 @@
 // te_inst.cu -- instantiates every kernel whose BRA pair class is TE_CB (compiled 10 times, -DTE_CB=0..9, so the
 // 55 (la lb|lc ld) classes build in parallel).  Exposes launch_*_cb<TE_CB> entry points used by te_dispatch.cu.
 #include "te_jkq.cuh"
+#include "te_jkb.cuh"
 
 #include <cstdlib>
 
@@ -48,12 +49,32 @@ static int jk_launch(te_pairs* P, double tau, int lane, cudaStream_t st) {
     a.tile_start = P->d_tile_start[lane]; a.ctrl = P->d_ctrl; a.tau = tau; a.nbf = b->nbf; a.nshells = b->nshells;
     a.slot = slot; a.same = (TE_CB == CK);
     a.task_hi = P->d_task_hi[lane];
+    a.bstart = P->d_bstart[TE_CB]; a.nblk = P->nblk[TE_CB];
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     // 0: generic thread-per-quartet kernel everywhere; 1: uniform-ket warp kernel for the non-light classes;
     // 2 (default): split-quartet kernel where instantiated (use_jkq), uniform-ket warp kernel for every other class
     static const int impl = getenv("TE_JK_IMPL") ? atoi(getenv("TE_JK_IMPL")) : 2;
+    if constexpr (use_jkb(LA, LB, LC, LD)) {
+        if (impl == 2 || impl == 4) {
+            // block-per-lane kernel for the s/p-only classes: one warp per block, ket tables in shared memory
+            using S = BShape<LA, LB, LC, LD>;
+            constexpr int smem = S::smem_doubles * (int)sizeof(double);
+            static int blocks_per_sm = 0;
+            if (!blocks_per_sm) {
+                TE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, jkb_kernel<LA, LB, LC, LD>, WARP, smem));
+                if (blocks_per_sm < 1) { blocks_per_sm = 0; set_error("jkb_kernel<%d,%d,%d,%d> does not fit", LA, LB, LC, LD); return TE_ERR_CUDA; }
+            }
+            const int warps = sms * blocks_per_sm;
+            schedule_w_kernel<<<1, 1024, 0, st>>>(P->d_qmax[TE_CB], a.nb, a.qk, a.nk, a.same, tau, warps, WARP, P->d_tile_start[lane], P->d_task_hi[lane], P->d_ctrl, slot);
+            const long long max_tasks = a.nk * ((a.nb + WARP - 1) / WARP);
+            const unsigned grid = (unsigned)std::min<long long>(max_tasks, (long long)warps);
+            jkb_kernel<LA, LB, LC, LD><<<grid, WARP, smem, st>>>(a);
+            TE_CUDA(cudaGetLastError());
+            return TE_OK;
+        }
+    }
     if constexpr (use_jkq(LA, LB, LC, LD)) {
         if (impl == 3 || (impl == 2 && jkq_default(LA, LB, LC, LD))) {
             constexpr int QW = 4, QG = jkq_lanes(LA, LB, LC, LD, QW);

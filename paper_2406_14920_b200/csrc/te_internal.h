@@ -63,6 +63,8 @@ struct te_pairs {
     double* d_qmax[TE_NCLASS] = {nullptr};   // largest bound of the pair's contracted shell-pair block (non-increasing along the list)
     te::PairIds* d_ids[TE_NCLASS] = {nullptr};
     // Hermite density / Hermite J of every pair (eq. 35), [count][nherm(la+lb)], rebuilt / zeroed by every build
+    int* d_bstart[TE_NCLASS] = {nullptr};   // first pair of every contracted shell-pair block, [nblk + 1]
+    int nblk[TE_NCLASS] = {0};
     double* d_DH[TE_NCLASS] = {nullptr};
     double* d_JH[TE_NCLASS] = {nullptr};
     // per-build scratch

@@ -222,6 +222,7 @@ struct JKArgs {
     const PairD* pk; const double* qk; const PairIds* ik; long long nk;
     const double* Ds; const double* Dm; double* Jt; double* Kt;
     const double* boys_tab;
+    const int* bstart; int nblk;            // first pair of every contracted shell-pair block of the bra list, [nblk + 1]
     const double* DHb; const double* DHk;   // Hermite densities of the bra / ket pair lists (split-quartet kernel)
     double* JHb; double* JHk;               // Hermite J accumulators of the bra / ket pair lists
     const long long* tile_start;

@@ -289,6 +289,17 @@ extern "C" int te_shellpair_build(const te_basis* b, double tau_pair, te_pairs**
                 cub::DeviceRadixSort::SortPairsDescending(tmp2, tb2, bm, P->d_qmax[cls], p1, p2, (int)nk);
                 permute_pairs_kernel<<<gr, 256>>>(p2, (long long)nk, t_pair, t_ids, d_qs, P->d_pair[cls], P->d_ids[cls], P->d_q[cls]);
                 cudaError_t e2 = cudaDeviceSynchronize();
+                if (e2 == cudaSuccess) {
+                    // block directory: where a new contracted shell pair starts in the final order
+                    std::vector<PairIds> hid(nk);
+                    e2 = cudaMemcpy(hid.data(), P->d_ids[cls], nk * sizeof(PairIds), cudaMemcpyDeviceToHost);
+                    std::vector<int> bs;
+                    for (unsigned long long x = 0; x < nk; ++x)
+                        if (x == 0 || hid[x].shA != hid[x - 1].shA || hid[x].shB != hid[x - 1].shB) bs.push_back((int)x);
+                    P->nblk[cls] = (int)bs.size();
+                    bs.push_back((int)nk);
+                    if (e2 == cudaSuccess && upload(bs, &P->d_bstart[cls]) != TE_OK) e2 = cudaErrorMemoryAllocation;
+                }
                 cleanup2();
                 if (e2 != cudaSuccess) { cleanup(); set_error("te_shellpair_build: %s", cudaGetErrorString(e2)); return fail(TE_ERR_CUDA); }
             }
@@ -325,7 +336,7 @@ extern "C" int te_shellpair_build(const te_basis* b, double tau_pair, te_pairs**
 
 extern "C" void te_pairs_destroy(te_pairs* P) {
     if (!P) return;
-    for (int c = 0; c < TE_NCLASS; ++c) { cudaFree(P->d_pair[c]); cudaFree(P->d_q[c]); cudaFree(P->d_ids[c]); cudaFree(P->d_DH[c]); cudaFree(P->d_JH[c]); cudaFree(P->d_qmax[c]); }
+    for (int c = 0; c < TE_NCLASS; ++c) { cudaFree(P->d_pair[c]); cudaFree(P->d_q[c]); cudaFree(P->d_ids[c]); cudaFree(P->d_DH[c]); cudaFree(P->d_JH[c]); cudaFree(P->d_qmax[c]); cudaFree(P->d_bstart[c]); }
     cudaFree(P->d_Ds); cudaFree(P->d_Jt); cudaFree(P->d_Kt); cudaFree(P->d_Dm); cudaFree(P->d_ctrl);
     for (int s = 0; s < te_pairs::NSTREAM; ++s) {
         cudaFree(P->d_tile_start[s]); cudaFree(P->d_task_hi[s]);
