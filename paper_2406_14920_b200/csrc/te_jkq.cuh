@@ -117,7 +117,7 @@ constexpr int jkq_smem(int la, int lb, int lc, int ld, int g, int w) {
 }
 constexpr int jkq_lanes(int la, int lb, int lc, int ld, int w) {
     const int nkl = ncart(lc) * ncart(ld);
-    int g = nkl >= 100 ? 16 : nkl >= 30 ? 8 : nkl >= 10 ? 4 : 2;
+    int g = nkl >= 100 ? 8 : nkl >= 30 ? 4 : 2;
     if (la + lb <= 3 && lc + ld <= 5) g = 2;   // measured: light bras gain 10 % from 16 quartets per warp ((PD|PF), (PD|DD))
     // blocks per SM are set by registers (launch bounds: 4 for light bras, 2 otherwise); shared memory may use the rest
     const int cap = nherm(la + lb) <= 10 ? 54 * 1024 : 110 * 1024;
