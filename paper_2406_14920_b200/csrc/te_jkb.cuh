@@ -213,7 +213,9 @@ __global__ void __launch_bounds__(WARP) jkb_kernel(JKArgs a) {
 #pragma unroll
                     for (int x = 0; x < NA * NC; ++x) dak[x] = 0.0;
                 }
-                if (live_jab | live_jcd | live_kac | live_kbc | live_kad | live_kbd) {
+                if (!(live_jab | live_jcd | live_kac | live_kbc | live_kad | live_kbd)) {
+                    cur = end;   // bounds fall along the block: the rest of it is dead too
+                } else {
                     ++nlive;
                     const PairD bp = a.pb[bi];
                     const PairIds ibp = a.ib[bi];
