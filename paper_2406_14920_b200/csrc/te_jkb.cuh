@@ -19,7 +19,7 @@ constexpr int jkb_outputs(int la, int lb, int lc, int ld) {
 // classes handled by the block-per-lane kernel: everything must fit in registers
 // (measured: (ss|ss) is faster with one primitive quartet per lane)
 constexpr bool use_jkb(int la, int lb, int lc, int ld) {
-    return la + lb + lc + ld >= 1 && la + lb + lc + ld <= 3 && jkb_outputs(la, lb, lc, ld) <= 31;
+    return la + lb + lc + ld >= 1 && la + lb + lc + ld <= 4 && jkb_outputs(la, lb, lc, ld) <= 39;
 }
 
 template <int LA, int LB, int LC, int LD>
