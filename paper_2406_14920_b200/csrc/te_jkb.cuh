@@ -16,10 +16,11 @@ namespace te {
 constexpr int jkb_outputs(int la, int lb, int lc, int ld) {
     return ncart(la) * ncart(lb) + (ncart(la) + ncart(lb)) * (ncart(lc) + ncart(ld));
 }
-// classes handled by the block-per-lane kernel: everything must fit in registers
-// (measured: (ss|ss) is faster with one primitive quartet per lane)
+// classes handled by the block-per-lane kernel: R (L <= 4: 35 values), the density blocks and all outputs of a quartet must fit
+// in registers (up to 48 outputs a few of them spill, still faster than the shared-memory R column of the uniform-ket kernel;
+// measured: (ss|ss) and (sd|sd) are faster with one primitive quartet per lane)
 constexpr bool use_jkb(int la, int lb, int lc, int ld) {
-    return la + lb + lc + ld >= 1 && la + lb + lc + ld <= 4 && jkb_outputs(la, lb, lc, ld) <= 39;
+    return la + lb + lc + ld >= 1 && la + lb + lc + ld <= 4 && jkb_outputs(la, lb, lc, ld) <= 48;
 }
 
 template <int LA, int LB, int LC, int LD>
