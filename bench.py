@@ -28,7 +28,7 @@ METRIC = "primitive_shell_quartets_per_s"
 UNIT = "quartets/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the class kernels captured with ncu --set full
 # (profiles/r1_ncu_full_final_cfg2.txt); other kernels / configs have no capture and report null
-NCU_DRAM_BYTES = {(2, "(SP|PD)"): 3.90e6, (2, "(SP|PF)"): 3.80e6, (2, "(PD|PF)"): 3.50e6}
+NCU_DRAM_BYTES = {(2, "(SP|DF)"): 3.61e6, (2, "(SP|PD)"): 5.70e6, (2, "(PD|PF)"): 3.52e6}
 CONFIG_NAMES = {1: "cfg1_tiny", 2: "cfg2_small_organic", 3: "cfg3_water16", 4: "cfg4_metal_complex",
                 5: "cfg5_large_organic"}
 
