@@ -45,6 +45,11 @@ def lib():
         L.orc_eri_shell_quartet.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_double)]
         L.orc_overlap_shell.argtypes = [C.c_void_p, C.c_int, C.c_int, C.POINTER(C.c_double)]
         L.orc_prim_eri_raw.argtypes = ([C.c_int, C.c_double, C.POINTER(C.c_double)] * 4) + [C.POINTER(C.c_double)]
+        L.orc_prim_eri_raw_lr.argtypes = ([C.c_int, C.c_double, C.POINTER(C.c_double)] * 4) + [C.c_double, C.POINTER(C.c_double)]
+        L.orc_set_omega.argtypes = [C.c_void_p, C.c_double]
+        L.orc_density_bounds.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.orc_nuclear_attraction.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double),
+                                             C.POINTER(C.c_double)]
         L.orc_num_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -64,11 +69,13 @@ def boys(mmax: int, T: float) -> np.ndarray:
     return F
 
 
-def prim_eri_raw(la, a, A, lb, b, B, lc, c, Cc, ld, d, Dd) -> np.ndarray:
-    """Block of UNNORMALISED primitive integrals (C_mu = 1), eq. 30; shape [nA,nB,nC,nD]."""
+def prim_eri_raw(la, a, A, lb, b, B, lc, c, Cc, ld, d, Dd, omega: float = 0.0) -> np.ndarray:
+    """Block of UNNORMALISED primitive integrals (C_mu = 1), shape [nA,nB,nC,nD]: eq. 30, or the
+    long-range erf(omega r)/r integrals of eq. 33 when omega > 0."""
     A, B, Cc, Dd = (np.ascontiguousarray(x, dtype=np.float64) for x in (A, B, Cc, Dd))
     out = np.zeros((ncart(la), ncart(lb), ncart(lc), ncart(ld)))
-    lib().orc_prim_eri_raw(la, float(a), _dp(A), lb, float(b), _dp(B), lc, float(c), _dp(Cc), ld, float(d), _dp(Dd), _dp(out))
+    lib().orc_prim_eri_raw_lr(la, float(a), _dp(A), lb, float(b), _dp(B), lc, float(c), _dp(Cc), ld, float(d), _dp(Dd),
+                              float(omega), _dp(out))
     return out
 
 
@@ -130,6 +137,25 @@ class Oracle:
         q = np.zeros(self.nprim * (self.nprim + 1) // 2)
         self.L.orc_all_bounds(self.ctx, _dp(q))
         return q
+
+    def set_omega(self, omega: float):
+        """Operator of the J/K builds: 0 = 1/r, omega > 0 = erf(omega r)/r (eq. 32-33).  Pair lists are unaffected."""
+        self.L.orc_set_omega(self.ctx, float(omega))
+
+    def density_bounds(self, D) -> np.ndarray:
+        """Dm[X][Y] = max |D| over the block of contracted shells (X,Y)."""
+        D = np.ascontiguousarray(D, dtype=np.float64)
+        Dm = np.zeros((self.nshells, self.nshells))
+        self.L.orc_density_bounds(self.ctx, _dp(D), _dp(Dm))
+        return Dm
+
+    def nuclear_attraction(self, xyz_c, q_c) -> np.ndarray:
+        """V_mu,nu = sum_C q_C (mu| 1/|r-C| |nu), eq. 14-26, over the kept primitive pairs (build_pairs first)."""
+        xyz_c = np.ascontiguousarray(xyz_c, dtype=np.float64).reshape(-1, 3)
+        q_c = np.ascontiguousarray(q_c, dtype=np.float64)
+        V = np.zeros((self.nbf, self.nbf))
+        self.L.orc_nuclear_attraction(self.ctx, len(q_c), _dp(xyz_c), _dp(q_c), _dp(V))
+        return V
 
     def jk_o2(self, D, tau: float):
         """Production oracle: symmetry-unique quartets + per-term screening.  Returns J, K, stats."""

@@ -12,8 +12,12 @@
  * Pins (tests/test_oracle_*.py): Boys vs scipy/mpmath incomplete gamma; unit self-overlap; closed-form
  * (ss|ss) eq. 28; brute-force Gauss-Hermite/Legendre quadrature of primitive integrals for every l;
  * 8-fold symmetry eq. 46; Schwarz inequality; translation / rotation invariance of Tr(DJ), Tr(DK);
- * O2 (symmetry-unique loops) == O1 (definition).  "parity unpinned": only the SIZE of the screening
- * error (no bound is printed in the paper); it is measured, not asserted.
+ * O2 (symmetry-unique loops) == O1 (definition); Schwarz bound eq. 45 against its definition written out in
+ * numpy and the (ss|ss) closed form; density bounds against a numpy block maximum; the per-term rule against a
+ * numpy transcription on a tiny basis; long-range integrals eq. 33 against the attenuated (ss|ss) closed form,
+ * the omega -> infinity limit and quadrature of eq. 32; nuclear attraction eq. 26 against eq. 17, 1-D
+ * quadrature and the tight-s-charge limit of the (pinned) ERI code.  "parity unpinned": only the SIZE of the
+ * screening error (no bound is printed in the paper); it is measured, not asserted.
  */
 #include <math.h>
 #include <stdlib.h>
@@ -97,6 +101,7 @@ typedef struct {
     long npairs;     /* kept, canonical (unordered) */
     OPair *pairs;
     double compf[NL][10];  /* per-component normalisation factor f(i) (step 1) */
+    double omega;          /* 0: full-range 1/r (eq. 30); > 0: long-range erf(omega r)/r (eq. 32-33) in the J/K builds */
 } OrcCtx;
 
 /* Step 1 (eq. 1-2; north_star "unit self-overlap"; reading 3).
@@ -245,18 +250,27 @@ static void r_table(int L, double alpha, const double X[3], RTab *Rp) {
  * out[((i*nB + j)*nC + k)*nD + l] = (m_i n_j | r_k s_l), all coefficient factors included
  * (C_mu of P:51 = c~ x f(i)).  Bracketing of eq. 31: inner_P = sum_Q E_Q^{kl} (-1)^Q R_{P+Q},
  * then sum_P E_P^{ij} inner_P; the prefactor 2 pi^{5/2} / (p q sqrt(p+q)) of eq. 30.
- * Ket E's take the ket exponent q (eq. 29; reading 2). */
-static void prim_block(const OrcCtx *c, const OPair *bra, const OPair *ket, double *out) {
+ * Ket E's take the ket exponent q (eq. 29; reading 2).
+ *
+ * Long-range operator erf(omega r)/r (eq. 32-33): identical sums; only the argument of the
+ * auxiliary integrals, alpha -> p q omega^2 / (p q + (p + q) omega^2), and the prefactor,
+ * 2 pi^{5/2} omega / (p q sqrt(p q + (p + q) omega^2)), change.  omega <= 0 selects the full-range eq. 30. */
+static void prim_block_op(const OrcCtx *c, const OPair *bra, const OPair *ket, double omega, double *out) {
     const int la = c->prim[bra->m].l, lb = c->prim[bra->n].l, lc = c->prim[ket->m].l, ld = c->prim[ket->n].l;
     const int nA = ncart(la), nB = ncart(lb), nC = ncart(lc), nD = ncart(ld);
     const int Lab = la + lb, Lcd = lc + ld, L = Lab + Lcd;
     const double p = bra->p, q = ket->p;
-    const double alpha = p * q / (p + q);
+    double alpha = p * q / (p + q);
+    double pref = 2.0 * pow(PI, 2.5) / (p * q * sqrt(p + q)) * bra->cc * ket->cc;
+    if (omega > 0.0) {   /* eq. 33 */
+        const double den = p * q + p * omega * omega + q * omega * omega;
+        alpha = p * q * omega * omega / den;
+        pref = 2.0 * pow(PI, 2.5) * omega / (p * q * sqrt(den)) * bra->cc * ket->cc;
+    }
     double X[3] = {bra->P[0] - ket->P[0], bra->P[1] - ket->P[1], bra->P[2] - ket->P[2]};
     static __thread RTab Rbuf;
     RTab *Rp = &Rbuf;
     r_table(L, alpha, X, Rp);
-    const double pref = 2.0 * pow(PI, 2.5) / (p * q * sqrt(p + q)) * bra->cc * ket->cc;
     const int szb = (la + 1) * (lb + 1) * (Lab + 1), szk = (lc + 1) * (ld + 1) * (Lcd + 1);
 #define EB(d, i, j, t) bra->E[(d) * szb + (((i) * (lb + 1) + (j)) * (Lab + 1)) + (t)]
 #define EK(d, i, j, t) ket->E[(d) * szk + (((i) * (ld + 1) + (j)) * (Lcd + 1)) + (t)]
@@ -297,9 +311,17 @@ static void prim_block(const OrcCtx *c, const OPair *bra, const OPair *ket, doub
 #undef EK
 }
 
-/* Raw primitive integral block for pins: unit coefficients (C = 1), arbitrary centres / exponents. */
-void orc_prim_eri_raw(int la, double a, const double *A, int lb, double b, const double *B,
-                      int lc, double cexp, const double *C, int ld, double d, const double *Dc, double *out) {
+/* Full-range block (eq. 30): what the Schwarz bounds, the pair lists and the integral-block checks use. */
+static void prim_block(const OrcCtx *c, const OPair *bra, const OPair *ket, double *out) { prim_block_op(c, bra, ket, 0.0, out); }
+
+/* Operator used by the J/K builds (orc_jk_o1 / orc_jk_o2): 0 = 1/r (default), omega > 0 = erf(omega r)/r.
+   Pair lists and Schwarz bounds stay those of the full-range operator (reading 20). */
+void orc_set_omega(OrcCtx *c, double omega) { c->omega = omega > 0.0 ? omega : 0.0; }
+
+/* Raw primitive integral block for pins: unit coefficients (C = 1), arbitrary centres / exponents;
+   omega <= 0: eq. 30, omega > 0: eq. 33. */
+void orc_prim_eri_raw_lr(int la, double a, const double *A, int lb, double b, const double *B,
+                         int lc, double cexp, const double *C, int ld, double d, const double *Dc, double omega, double *out) {
     OrcCtx ctx; memset(&ctx, 0, sizeof(ctx));
     OPrim pr[4];
     const int ls[4] = {la, lb, lc, ld}; const double es[4] = {a, b, cexp, d}; const double *cs[4] = {A, B, C, Dc};
@@ -307,8 +329,13 @@ void orc_prim_eri_raw(int la, double a, const double *A, int lb, double b, const
     ctx.prim = pr; ctx.nprim = 4;
     for (int l = 0; l < NL; ++l) for (int i = 0; i < 10; ++i) ctx.compf[l][i] = 1.0;
     OPair bra, ket; make_pair(&ctx, 0, 1, &bra); make_pair(&ctx, 2, 3, &ket);
-    prim_block(&ctx, &bra, &ket, out);
+    prim_block_op(&ctx, &bra, &ket, omega, out);
     free(bra.E); free(ket.E);
+}
+
+void orc_prim_eri_raw(int la, double a, const double *A, int lb, double b, const double *B,
+                      int lc, double cexp, const double *C, int ld, double d, const double *Dc, double *out) {
+    orc_prim_eri_raw_lr(la, a, A, lb, b, B, lc, cexp, C, ld, d, Dc, 0.0, out);
 }
 
 /* Overlap block of two contracted shells by eq. 11: S = C C E0x E0y E0z (pi/p)^{3/2}. */
@@ -437,6 +464,12 @@ static double *density_bounds(const OrcCtx *c, const double *D) {
     return Dm;
 }
 
+void orc_density_bounds(const OrcCtx *c, const double *D, double *Dm_out) {
+    double *Dm = density_bounds(c, D);
+    memcpy(Dm_out, Dm, sizeof(double) * (size_t)c->nshells * c->nshells);
+    free(Dm);
+}
+
 /* ------------------------------------------------------------------- O1: J and K from the definition
  * Eq. 34 and eq. 36 over ORDERED primitive pairs of the kept set, no permutational
  * symmetry, with the per-term rule of eq. 47 (readings 6, 8):
@@ -486,7 +519,7 @@ void orc_jk_o1(const OrcCtx *c, const double *D, double tau, double *J, double *
                 const int liveK = doK && (qq * Dm[B * ns + Dd] >= tau);
                 if (!liveJ && !liveK) continue;
                 const int nC = ncart(pr->l), nD = ncart(ps->l), oC = c->shell_off[C], oD = c->shell_off[Dd];
-                prim_block(c, bra, ket, blk);
+                prim_block_op(c, bra, ket, c->omega, blk);
                 for (int i = 0; i < nA; ++i)
                     for (int j = 0; j < nB; ++j)
                         for (int k = 0; k < nC; ++k)
@@ -521,7 +554,7 @@ void orc_jk_o2(const OrcCtx *c, const double *D, double tau, double *J, double *
 #ifdef _OPENMP
     nth = omp_get_max_threads();
 #endif
-    double **Jt = (double **)malloc(sizeof(double *) * nth), **Kt = (double **)malloc(sizeof(double *) * nth);
+    double **Jt = (double **)calloc(nth, sizeof(double *)), **Kt = (double **)calloc(nth, sizeof(double *));   /* NULL = thread never ran */
     long long nlive = 0, nvis = 0, nborder = 0;
 #pragma omp parallel reduction(+ : nlive, nvis, nborder)
     {
@@ -555,7 +588,7 @@ void orc_jk_o2(const OrcCtx *c, const double *D, double tau, double *J, double *
                 if (!any) continue;
                 ++nlive;
                 const int nC = ncart(pr->l), nD = ncart(ps->l), oC = c->shell_off[C], oD = c->shell_off[Dd];
-                prim_block(c, bra, ket, blk);
+                prim_block_op(c, bra, ket, c->omega, blk);
                 double f = 1.0;
                 if (bra->m == bra->n) f *= 0.5;
                 if (ket->m == ket->n) f *= 0.5;
@@ -611,6 +644,46 @@ void orc_eri_shell_quartet(const OrcCtx *c, int A, int B, int C, int Dd, double 
             free(bra.E);
         }
     free(blk);
+}
+
+/* ------------------------------------------------------------ nuclear attraction V_mu,nu (eq. 14-26)
+ * V_mu,nu = sum_C V_mu,nu,C (eq. 16), V_mu,nu,C = q_C C_mu C_nu (2 pi / p) sum_tuv E_t E_u E_v R^0_tuv(p, P - C)
+ * (eq. 26), over the KEPT primitive shell pairs ("one primitive shell pair to one GPU thread ...
+ * every thread loop through all point charges"); the operator is + q_C / |r - C| as printed in eq. 14 (a nucleus
+ * of charge Z enters with q_C = -Z).  V is nbf x nbf, symmetric, overwritten.  orc_build_pairs must have run. */
+void orc_nuclear_attraction(const OrcCtx *c, int ncharge, const double *xyzC, const double *qC, double *V) {
+    const int nbf = c->nbf;
+    memset(V, 0, sizeof(double) * (size_t)nbf * nbf);
+    RTab *Rp = (RTab *)malloc(sizeof(RTab));
+    for (long I = 0; I < c->npairs; ++I) {
+        const OPair *pr = &c->pairs[I];
+        const OPrim *pm = &c->prim[pr->m], *pn = &c->prim[pr->n];
+        const int la = pm->l, lb = pn->l, nA = ncart(la), nB = ncart(lb), Lab = la + lb;
+        const int oA = c->shell_off[pm->shell], oB = c->shell_off[pn->shell];
+        const int szb = (la + 1) * (lb + 1) * (Lab + 1);
+        for (int C = 0; C < ncharge; ++C) {
+            double X[3] = {pr->P[0] - xyzC[3 * C], pr->P[1] - xyzC[3 * C + 1], pr->P[2] - xyzC[3 * C + 2]};
+            r_table(Lab, pr->p, X, Rp);
+            for (int i = 0; i < nA; ++i) {
+                int ci[3]; cart_comp(la, i, ci);
+                for (int j = 0; j < nB; ++j) {
+                    int cj[3]; cart_comp(lb, j, cj);
+                    double s = 0.0;
+                    for (int t = 0; t <= ci[0] + cj[0]; ++t)
+                        for (int u = 0; u <= ci[1] + cj[1]; ++u)
+                            for (int v = 0; v <= ci[2] + cj[2]; ++v)
+                                s += pr->E[0 * szb + ((ci[0] * (lb + 1) + cj[0]) * (Lab + 1)) + t] *
+                                     pr->E[1 * szb + ((ci[1] * (lb + 1) + cj[1]) * (Lab + 1)) + u] *
+                                     pr->E[2 * szb + ((ci[2] * (lb + 1) + cj[2]) * (Lab + 1)) + v] * (*Rp)[0][t][u][v];
+                    const double val = qC[C] * pr->cc * c->compf[la][i] * c->compf[lb][j] * (2.0 * PI / pr->p) * s;
+                    V[(long)(oA + i) * nbf + oB + j] += val;
+                    /* the unordered pair (m,n), m != n, stands for both ordered pairs: mirror element */
+                    if (pr->m != pr->n) V[(long)(oB + j) * nbf + oA + i] += val;
+                }
+            }
+        }
+    }
+    free(Rp);
 }
 
 int orc_num_threads(void) {

@@ -22,7 +22,8 @@ FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-li
 
 
 def _deps_mtime() -> float:
-    files = glob.glob(os.path.join(CSRC, "*")) + [os.path.join(HERE, "..", "include", "te_jk.h")]
+    files = [f for pat in ("*.cu", "*.cuh", "*.h") for f in glob.glob(os.path.join(CSRC, pat))]
+    files.append(os.path.join(HERE, "..", "include", "te_jk.h"))
     return max(os.path.getmtime(f) for f in files)
 
 

@@ -4,7 +4,7 @@
     1/r12 = (2/sqrt(pi)) int_0^inf exp(-u^2 r12^2) du ;
 
 for each u the 6-D integral factorises into three 2-D integrals over (x1, x2) of
-polynomial x exp(-quadratic form); each is done EXACTLY by a 12x12 Gauss-Hermite rule in the eigenbasis
+polynomial x exp(-quadratic form); each is done EXACTLY by a 14x14 Gauss-Hermite rule in the eigenbasis
 of the quadratic form [[p+u^2, -u^2], [-u^2, q+u^2]], and the outer u integral by Gauss-Legendre in t with
 u = sqrt(rho) t / sqrt(1-t^2), rho = pq/(p+q).  Pure numpy; test helper only.
 """
@@ -37,18 +37,45 @@ def _dim_integral(u, i, a, A, j, b, B, k, c, C, l, d, D):
     return out
 
 
-def eri_quadrature(ia, a, A, ib, b, B, ic, c, C, id_, d, D, nodes=120):
-    """(mu nu | lambda sigma) for unnormalised primitives with Cartesian powers ia, ib, ic, id_ (3-tuples)."""
+def eri_quadrature(ia, a, A, ib, b, B, ic, c, C, id_, d, D, nodes=120, omega=None):
+    """(mu nu | lambda sigma) for unnormalised primitives with Cartesian powers ia, ib, ic, id_ (3-tuples).
+    omega: long-range operator erf(omega r)/r = (2/sqrt(pi)) int_0^omega exp(-u^2 r^2) du (eq. 32, PAPER.md
+    line 222): the same integrand, the outer integral simply stops at u = omega."""
     p, q = a + b, c + d
     rho = p * q / (p + q)
     x, w = np.polynomial.legendre.leggauss(nodes)
-    t = 0.5 * (x + 1.0)
-    w = 0.5 * w
+    tmax = 1.0 if omega is None else omega / np.sqrt(rho + omega * omega)   # u = omega  <=>  t = tmax
+    t = 0.5 * tmax * (x + 1.0)
+    w = 0.5 * tmax * w
     u = np.sqrt(rho) * t / np.sqrt(1.0 - t * t)
     du = np.sqrt(rho) * (1.0 - t * t) ** (-1.5)
     f = np.ones_like(u)
     for dim in range(3):
         f = f * _dim_integral(u, ia[dim], a, A[dim], ib[dim], b, B[dim], ic[dim], c, C[dim], id_[dim], d, D[dim])
+    return 2.0 / np.sqrt(np.pi) * np.sum(w * du * f)
+
+
+def nuclear_quadrature(ia, a, A, ib, b, B, C, nodes=160):
+    """int mu(r) nu(r) / |r - C| dr for unnormalised primitives (eq. 15, q_C = 1), with
+    1/|r-C| = (2/sqrt(pi)) int_0^inf exp(-u^2 |r-C|^2) du: per u three 1-D integrals of polynomial x Gaussian,
+    each exact by Gauss-Hermite; outer integral by Gauss-Legendre in t, u = sqrt(p) t / sqrt(1 - t^2)."""
+    p = a + b
+    x, w = np.polynomial.legendre.leggauss(nodes)
+    t = 0.5 * (x + 1.0)
+    w = 0.5 * w
+    u = np.sqrt(p) * t / np.sqrt(1.0 - t * t)
+    du = np.sqrt(p) * (1.0 - t * t) ** (-1.5)
+    f = np.ones_like(u)
+    for dim in range(3):
+        Ax, Bx, Cx, i, j = A[dim], B[dim], C[dim], ia[dim], ib[dim]
+        g = np.empty_like(u)
+        for n, uu in enumerate(u):
+            s_ = p + uu * uu                                  # exponent of the product Gaussian
+            x0 = (a * Ax + b * Bx + uu * uu * Cx) / s_
+            c0 = a * Ax * Ax + b * Bx * Bx + uu * uu * Cx * Cx - s_ * x0 * x0
+            xs = x0 + _GH_X / np.sqrt(s_)
+            g[n] = np.exp(-c0) * np.sum(_GH_W * (xs - Ax) ** i * (xs - Bx) ** j) / np.sqrt(s_)
+        f = f * g
     return 2.0 / np.sqrt(np.pi) * np.sum(w * du * f)
 
 
