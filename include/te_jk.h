@@ -86,6 +86,12 @@ int te_build_jk_host(const te_pairs *p, const double *D_host, double *J_host, do
  * indexed [bra class][ket class] (only bra class <= ket class is used): unique primitive quartets that
  * had at least one live update, and device milliseconds spent in that class pair's kernel. */
 int te_jk_stats(const te_pairs *p, long long quartets[TE_NCLASS][TE_NCLASS], float ms[TE_NCLASS][TE_NCLASS]);
+/* Screening statistics of the LAST te_build_jk on this handle (synchronises), same indexing: `visited` = unique
+ * primitive quartets inside the schedule's cut whose per-term tests (eq. 47) were evaluated (the oracle's
+ * "visited" counts every unique quartet of the kept lists; the cut of P:391 skips the rest), `slots` = quartet
+ * slots of the warp batches that ran the integral code, so live / slots is the lane occupancy of the class kernel.
+ * Either pointer may be NULL. */
+int te_jk_screening_stats(const te_pairs *p, long long visited[TE_NCLASS][TE_NCLASS], long long slots[TE_NCLASS][TE_NCLASS]);
 /* Enable (1) / disable (0) per-class CUDA-event timing for te_jk_stats (off by default). */
 int te_jk_set_profiling(te_pairs *p, int on);
 

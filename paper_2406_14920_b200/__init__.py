@@ -62,6 +62,7 @@ def lib():
     L.te_build_jk.argtypes = [vp, vp, vp, vp, C.c_double, vp]
     L.te_build_jk_host.argtypes = [vp, dpp, dpp, dpp, C.c_double]
     L.te_jk_stats.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_float)]
+    L.te_jk_screening_stats.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
     L.te_jk_set_profiling.argtypes = [vp, C.c_int]
     L.te_eri_block.argtypes = [vp, C.c_int, ipp, C.POINTER(C.c_longlong), vp]
     L.te_boys.argtypes = [C.c_int, vp, C.c_int, vp]
@@ -207,6 +208,14 @@ class Pairs:
         _check(lib().te_jk_stats(self.handle, q.ctypes.data_as(C.POINTER(C.c_longlong)),
                                  ms.ctypes.data_as(C.POINTER(C.c_float))), "te_jk_stats")
         return q, ms
+
+    def screening_stats(self):
+        """(visited[10][10], slots[10][10]) of the last build (te_jk_screening_stats)."""
+        v = np.zeros((NCLASS, NCLASS), dtype=np.int64)
+        s = np.zeros((NCLASS, NCLASS), dtype=np.int64)
+        _check(lib().te_jk_screening_stats(self.handle, v.ctypes.data_as(C.POINTER(C.c_longlong)),
+                                           s.ctypes.data_as(C.POINTER(C.c_longlong))), "te_jk_screening_stats")
+        return v, s
 
     def close(self):
         if getattr(self, "handle", None):

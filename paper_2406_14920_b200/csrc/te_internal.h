@@ -29,6 +29,8 @@ struct PairIds {
 struct JKControl {
     double dmax;                                        // max |D| (set by density_bounds_kernel)
     unsigned long long live[TE_NCLASS * TE_NCLASS];     // unique live quartets per class pair
+    unsigned long long visited[TE_NCLASS * TE_NCLASS];  // unique quartets whose eq. 47 tests were evaluated (inside the schedule's cut)
+    unsigned long long slots[TE_NCLASS * TE_NCLASS];    // quartet slots of the warp batches that ran the integral code (lane occupancy = live / slots)
     unsigned long long ntiles[TE_NCLASS * TE_NCLASS];   // scheduled tiles per class pair
     unsigned int tile_counter[TE_NCLASS * TE_NCLASS];   // dynamic tile queue heads
     int chunk[TE_NCLASS * TE_NCLASS];                   // uniform-ket kernel: bras per task = 32 * chunk

@@ -51,7 +51,7 @@ __global__ void __launch_bounds__(WARP) jkb_kernel(JKArgs a) {
     PairD kp;
     PairIds ik;
     double qk = 0.0, dm_jab = 0.0;
-    unsigned int nlive = 0;
+    unsigned int nlive = 0, nvis = 0, nslot = 0;
 
     while (true) {
         unsigned int task = 0;
@@ -187,7 +187,9 @@ __global__ void __launch_bounds__(WARP) jkb_kernel(JKArgs a) {
             nb += __popc(needm);
             const bool work = cur < end;
             if (!__any_sync(FULLMASK, work)) break;
+            ++nslot;
             if (work) {
+                ++nvis;
                 const long long bi = cur++;
                 const double qq = a.qb[bi] * qk;
                 // the per-term tests of eq. 47; bounds fall along the block, so a dead term stays dead: zero its density block
@@ -311,8 +313,14 @@ __global__ void __launch_bounds__(WARP) jkb_kernel(JKArgs a) {
         }
     }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) nlive += __shfl_down_sync(FULLMASK, nlive, o);
-    if (lane == 0 && nlive) atomicAdd(&a.ctrl->live[a.slot], (unsigned long long)nlive);
+    for (int o = 16; o > 0; o >>= 1) {
+        nlive += __shfl_down_sync(FULLMASK, nlive, o); nvis += __shfl_down_sync(FULLMASK, nvis, o); nslot += __shfl_down_sync(FULLMASK, nslot, o);
+    }
+    if (lane == 0 && nvis) {
+        atomicAdd(&a.ctrl->live[a.slot], (unsigned long long)nlive);
+        atomicAdd(&a.ctrl->visited[a.slot], (unsigned long long)nvis);
+        atomicAdd(&a.ctrl->slots[a.slot], (unsigned long long)nslot);
+    }
 }
 
 }  // namespace te

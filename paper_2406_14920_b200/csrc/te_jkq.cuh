@@ -175,7 +175,7 @@ __global__ void __launch_bounds__(32 * W, (nherm(LA + LB) <= 10 ? 4 : 2)) jkq_ke
     PairD kp;
     PairIds ik;
     double qk = 0.0;
-    unsigned int nlive = 0;
+    unsigned int nlive = 0, nvis = 0, nslot = 0;
 
     while (true) {
         if (tid == 0) s_task = atomicAdd(&a.ctrl->tile_counter[a.slot], 1u);
@@ -234,6 +234,7 @@ __global__ void __launch_bounds__(32 * W, (nherm(LA + LB) <= 10 ? 4 : 2)) jkq_ke
             PairIds ib;
             bool live_jab = false, live_jcd = false, live_kac = false, live_kbc = false, live_kad = false, live_kbd = false;
             if (active) {
+                if (g == 0) ++nvis;
                 ib = a.ib[bi];
                 const double qq = a.qb[bi] * qk;
                 live_jab = qq * a.Dm[ik.shA * ns + ik.shB] >= a.tau;
@@ -245,6 +246,7 @@ __global__ void __launch_bounds__(32 * W, (nherm(LA + LB) <= 10 ? 4 : 2)) jkq_ke
                 active = live_jab | live_jcd | live_kac | live_kbc | live_kad | live_kbd;
             }
             if (!__any_sync(FULLMASK, active)) continue;
+            if (g == 0) ++nslot;
             const bool any_jcd = __any_sync(FULLMASK, live_jcd);
             any_jcd_task |= any_jcd;
             const bool live_k = live_kac | live_kbc | live_kad | live_kbd;
@@ -445,8 +447,14 @@ __global__ void __launch_bounds__(32 * W, (nherm(LA + LB) <= 10 ? 4 : 2)) jkq_ke
         }
     }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) nlive += __shfl_down_sync(FULLMASK, nlive, o);
-    if (lane == 0 && nlive) atomicAdd(&a.ctrl->live[a.slot], (unsigned long long)nlive);
+    for (int o = 16; o > 0; o >>= 1) {
+        nlive += __shfl_down_sync(FULLMASK, nlive, o); nvis += __shfl_down_sync(FULLMASK, nvis, o); nslot += __shfl_down_sync(FULLMASK, nslot, o);
+    }
+    if (lane == 0 && nvis) {
+        atomicAdd(&a.ctrl->live[a.slot], (unsigned long long)nlive);
+        atomicAdd(&a.ctrl->visited[a.slot], (unsigned long long)nvis);
+        atomicAdd(&a.ctrl->slots[a.slot], (unsigned long long)nslot);
+    }
 }
 
 // ------------------------------------------------------------------- Hermite density / Hermite J (eq. 35)

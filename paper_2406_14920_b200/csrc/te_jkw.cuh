@@ -120,7 +120,7 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
     PairD kp;
     PairIds ik;
     double qk = 0.0;
-    unsigned int nlive = 0;
+    unsigned int nlive = 0, nvis = 0, nslot = 0;
 
     while (true) {
         unsigned int task = 0;
@@ -176,6 +176,7 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
             PairIds ib;
             bool live_jab = false, live_jcd = false, live_kac = false, live_kbc = false, live_kad = false, live_kbd = false;
             if (active) {
+                ++nvis;
                 ib = a.ib[bi];
                 const double qq = a.qb[bi] * qk;
                 live_jab = qq * a.Dm[ik.shA * ns + ik.shB] >= a.tau;
@@ -187,6 +188,7 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                 active = live_jab | live_jcd | live_kac | live_kbc | live_kad | live_kbd;
             }
             if (!__any_sync(FULLMASK, active)) continue;
+            ++nslot;
             const bool any_jcd = __any_sync(FULLMASK, live_jcd);
             // Runs of lanes whose bras are primitive pairs of ONE contracted shell pair (the lists are shell-pair-major) share every
             // bra-side output address: their contributions are summed by a segmented shuffle reduction and the run's first lane
@@ -416,8 +418,14 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
         }
     }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) nlive += __shfl_down_sync(FULLMASK, nlive, o);
-    if (lane == 0 && nlive) atomicAdd(&a.ctrl->live[a.slot], (unsigned long long)nlive);
+    for (int o = 16; o > 0; o >>= 1) {
+        nlive += __shfl_down_sync(FULLMASK, nlive, o); nvis += __shfl_down_sync(FULLMASK, nvis, o); nslot += __shfl_down_sync(FULLMASK, nslot, o);
+    }
+    if (lane == 0 && nvis) {
+        atomicAdd(&a.ctrl->live[a.slot], (unsigned long long)nlive);
+        atomicAdd(&a.ctrl->visited[a.slot], (unsigned long long)nvis);
+        atomicAdd(&a.ctrl->slots[a.slot], (unsigned long long)nslot);
+    }
 }
 
 // Task schedule of the uniform-ket kernel.  For ket j the live bras are a contiguous range of the (bound-sorted) bra list:

@@ -553,6 +553,19 @@ extern "C" int te_jk_stats(const te_pairs* P, long long quartets[TE_NCLASS][TE_N
     return TE_OK;
 }
 
+extern "C" int te_jk_screening_stats(const te_pairs* P, long long visited[TE_NCLASS][TE_NCLASS], long long slots[TE_NCLASS][TE_NCLASS]) {
+    if (!P) { set_error("te_jk_screening_stats: NULL handle"); return TE_ERR_BAD_ARG; }
+    TE_CUDA(cudaStreamSynchronize(P->last_stream));
+    JKControl h;
+    TE_CUDA(cudaMemcpy(&h, P->d_ctrl, sizeof(h), cudaMemcpyDeviceToHost));
+    for (int cb = 0; cb < TE_NCLASS; ++cb)
+        for (int ck = 0; ck < TE_NCLASS; ++ck) {
+            if (visited) visited[cb][ck] = (long long)h.visited[cb * TE_NCLASS + ck];
+            if (slots) slots[cb][ck] = (long long)h.slots[cb * TE_NCLASS + ck];
+        }
+    return TE_OK;
+}
+
 // ============================================================================================= utilities
 extern "C" int te_eri_block(const te_basis* b, int nq, const int* quartets, const long long* offs, double* out_dev) {
     if (!b || nq < 0 || (nq > 0 && (!quartets || !offs || !out_dev))) { set_error("te_eri_block: NULL argument"); return TE_ERR_BAD_ARG; }
