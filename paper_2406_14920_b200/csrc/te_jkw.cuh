@@ -55,8 +55,38 @@ struct WShape {
     // (4x more resident warps) made (DF|DF) 2.4x SLOWER -- these kernels are bound by per-warp instruction / local-memory
     // throughput, not by latency -- so every lane holds a quartet.
     static constexpr int NL = 32;
-    static constexpr int smem_doubles = NR * NL + NNZK + 3 * NE1 + NC * ND;
+    // without KEEPC the K_?c accumulators of the quartet live in a lane-private shared-memory column ((NA + NB) * NC values per
+    // lane): they are summed over l there and flushed ONCE per quartet instead of once per (k,l)
+    static constexpr int NKC = KEEPC ? 0 : (NA + NB) * NC;
+    static constexpr int smem_doubles = NR * NL + NNZK + 3 * NE1 + NC * ND + NKC * NL;
 };
+
+// Segmented reduction over runs of lanes + one atomic per run and value, for N values that share a live flag.  The shuffle
+// rounds of the N values are independent, so their latencies overlap (one value at a time, the rounds of a reduction form a
+// serial SHFL -> DADD chain of ~40 cycles each; measured: the per-value version was the largest single cost of this kernel).
+template <int N, class AddrFn>
+__device__ __forceinline__ void flush_vec(bool runs, int maxdist, int dist, bool head, bool live, double (&v)[N], AddrFn addr) {
+    constexpr unsigned FULLMASK = 0xffffffffu;
+    if (runs) {
+#pragma unroll
+        for (int x = 0; x < N; ++x) v[x] = live ? v[x] : 0.0;
+        for (int o = 1; o < maxdist; o <<= 1) {
+#pragma unroll
+            for (int x = 0; x < N; ++x) {
+                const double t = __shfl_down_sync(FULLMASK, v[x], o);
+                if (o < dist) v[x] += t;
+            }
+        }
+        if (head) {
+#pragma unroll
+            for (int x = 0; x < N; ++x)
+                if (v[x] != 0.0) atomicAdd(addr(x), v[x]);
+        }
+    } else if (live) {
+#pragma unroll
+        for (int x = 0; x < N; ++x) atomicAdd(addr(x), v[x]);
+    }
+}
 
 // R^0_{tuv} of eq. 21-25 built in place in a shared-memory column (element i at R[i * 32]); same sweep as rtable<L>.
 template <int L, int RS>
@@ -111,6 +141,7 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
     double* const dcd = e1 + 3 * S::NE1;
     const int lane = threadIdx.x;
     double* const Rl = Rsm + (lane < NL ? lane : 0);   // lanes >= NL never hold a quartet
+    double* const kcl = dcd + NC * ND + lane;          // K_?c accumulator column of this lane (only without KEEPC)
 
     const unsigned long long ntasks = a.ctrl->ntiles[a.slot];
     const long long span = (long long)NL * a.ctrl->chunk[a.slot];
@@ -201,18 +232,6 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
             const int dist = (above ? __ffs(above) - 1 : 32) - lane;
             const int maxdist = __reduce_max_sync(FULLMASK, dist);
             const bool runs = maxdist > 1;   // warp-uniform: without runs every lane adds its own contribution directly
-            auto flush = [&](bool live, double v, double* addr) {
-                if (runs) {
-                    v = live ? v : 0.0;
-                    for (int o = 1; o < maxdist; o <<= 1) {
-                        const double t = __shfl_down_sync(FULLMASK, v, o);
-                        if (o < dist) v += t;
-                    }
-                    if (head && v != 0.0) atomicAdd(addr, v);
-                } else if (live) {
-                    atomicAdd(addr, v);
-                }
-            };
             double f = 1.0;
             double Ebx[LA + 1][LB + 1][LAB + 1], Eby[LA + 1][LB + 1][LAB + 1], Ebz[LA + 1][LB + 1][LAB + 1];
             double dab[NA * NB], jab[NA * NB];
@@ -224,6 +243,9 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                 for (int x = 0; x < NA * NC; ++x) kac[x] = 0.0;
 #pragma unroll
                 for (int x = 0; x < NB * NC; ++x) kbc[x] = 0.0;
+            } else {
+#pragma unroll
+                for (int x = 0; x < S::NKC; ++x) kcl[x * NL] = 0.0;
             }
             const double* Da = nullptr; const double* Db = nullptr;   // rows of the scaled density at the bra's AOs
             if (active) {
@@ -382,11 +404,11 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                         }
                         if (!live_jcd) jkl = 0.0;
                     }
-                    if (!KEEPC) {
+                    if (!KEEPC) {   // sum over l in the lane's shared-memory column (inactive lanes add zeros)
 #pragma unroll
-                        for (int i = 0; i < NA; ++i) flush(live_kac, kak[i], &a.Kt[(ib.offA + i) * nbf + ik.offA + k]);
+                        for (int i = 0; i < NA; ++i) kcl[(i * NC + k) * NL] += kak[i];
 #pragma unroll
-                        for (int jj = 0; jj < NB; ++jj) flush(live_kbc, kbk[jj], &a.Kt[(ib.offB + jj) * nbf + ik.offA + k]);
+                        for (int jj = 0; jj < NB; ++jj) kcl[(NA * NC + jj * NC + k) * NL] += kbk[jj];
                     }
                     ptr += (sx + 1) * (sy + 1) * (sz + 1);
                     if (any_jcd) {
@@ -395,24 +417,25 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                         if (lane == 0) atomicAdd(&a.Jt[(ik.offA + k) * nbf + ik.offB + l], 2.0 * jkl);
                     }
                 }
-#pragma unroll
-                for (int i = 0; i < NA; ++i) flush(live_kad, kal[i], &a.Kt[(ib.offA + i) * nbf + ik.offB + l]);
-#pragma unroll
-                for (int jj = 0; jj < NB; ++jj) flush(live_kbd, kbl[jj], &a.Kt[(ib.offB + jj) * nbf + ik.offB + l]);
+                flush_vec<NA>(runs, maxdist, dist, head, live_kad, kal, [&](int i) { return &a.Kt[(ib.offA + i) * nbf + ik.offB + l]; });
+                flush_vec<NB>(runs, maxdist, dist, head, live_kbd, kbl, [&](int jj) { return &a.Kt[(ib.offB + jj) * nbf + ik.offB + l]; });
             }
 #pragma unroll
-            for (int i = 0; i < NA; ++i)
-#pragma unroll
-                for (int jj = 0; jj < NB; ++jj) flush(live_jab, 2.0 * jab[i * NB + jj], &a.Jt[(ib.offA + i) * nbf + ib.offB + jj]);
+            for (int x = 0; x < NA * NB; ++x) jab[x] *= 2.0;
+            flush_vec<NA * NB>(runs, maxdist, dist, head, live_jab, jab, [&](int x) { return &a.Jt[(ib.offA + x / NB) * nbf + ib.offB + x % NB]; });
             if (KEEPC) {
+                flush_vec<(KEEPC ? NA * NC : 1)>(runs, maxdist, dist, head, live_kac, kac, [&](int x) { return &a.Kt[(ib.offA + x / NC) * nbf + ik.offA + x % NC]; });
+                flush_vec<(KEEPC ? NB * NC : 1)>(runs, maxdist, dist, head, live_kbc, kbc, [&](int x) { return &a.Kt[(ib.offB + x / NC) * nbf + ik.offA + x % NC]; });
+            } else {
+                // the quartet's K_ac / K_bc sums come back from the shared-memory column, NC values (one row of the block) at a time
+#pragma unroll 1
+                for (int r = 0; r < NA + NB; ++r) {
+                    double row[NC];
 #pragma unroll
-                for (int i = 0; i < NA; ++i)
-#pragma unroll
-                    for (int k = 0; k < NC; ++k) flush(live_kac, kac[i * NC + k], &a.Kt[(ib.offA + i) * nbf + ik.offA + k]);
-#pragma unroll
-                for (int jj = 0; jj < NB; ++jj)
-#pragma unroll
-                    for (int k = 0; k < NC; ++k) flush(live_kbc, kbc[jj * NC + k], &a.Kt[(ib.offB + jj) * nbf + ik.offA + k]);
+                    for (int k = 0; k < NC; ++k) row[k] = kcl[(r * NC + k) * NL];
+                    const long long o1 = (r < NA ? ib.offA + r : ib.offB + (r - NA));
+                    flush_vec<NC>(runs, maxdist, dist, head, r < NA ? live_kac : live_kbc, row, [&](int k) { return &a.Kt[o1 * nbf + ik.offA + k]; });
+                }
             }
             __syncwarp();
         }
