@@ -3,9 +3,10 @@
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
 
-A "step" = one te_build_jk over one config (pair lists prebuilt, D resident in HBM).  Metric: unique primitive
-shell quartets per second (BASELINE.json: "shell-quartet ERIs/s"), with s/iter and the fraction of the measured
-FP64 FMA peak alongside.  N > 1 runs N independent replicas (the path does not shard: DESIGN.md section 8),
+A "step" = one te_build_jk over one config (pair lists prebuilt, D resident in HBM).  The default workload is
+config 5, the largest one (BASELINE.json north_star: "the largest config's J/K build"); --config 1..4 select the
+others.  Metric: unique primitive shell quartets per second (BASELINE.json: "shell-quartet ERIs/s"), with s/iter and
+the fraction of the measured FP64 FMA peak alongside.  N > 1 runs N independent replicas (the path does not shard: DESIGN.md section 8),
 timed as the max over ranks.  Prints ONE JSON line on rank 0.
 """
 from __future__ import annotations
@@ -26,9 +27,19 @@ import numpy as np  # noqa: E402
 
 METRIC = "primitive_shell_quartets_per_s"
 UNIT = "quartets/s"
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the class kernels captured with ncu --set full
-# (profiles/r1_ncu_full_final_cfg2.txt); other kernels / configs have no capture and report null
-NCU_DRAM_BYTES = {(2, "(SP|DF)"): 3.61e6, (2, "(SP|PD)"): 5.70e6, (2, "(PD|PF)"): 3.52e6}
+# roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch of a class kernel, taken from a committed
+# `ncu --set full` capture of THIS config (profiles/r2_dram_bytes.json: {"<config>": {"(AB|CD)": bytes}}, written from the
+# capture named inside that file); a class / config without a capture reports null
+DRAM_BYTES_FILE = os.path.join(ROOT, "profiles", "r2_dram_bytes.json")
+
+
+def ncu_dram_bytes(cfg: int, cls: str):
+    try:
+        with open(DRAM_BYTES_FILE) as fh:
+            return json.load(fh).get(str(cfg), {}).get(cls)
+    except (OSError, ValueError):
+        return None
+
 CONFIG_NAMES = {1: "cfg1_tiny", 2: "cfg2_small_organic", 3: "cfg3_water16", 4: "cfg4_metal_complex",
                 5: "cfg5_large_organic"}
 
@@ -122,8 +133,9 @@ def oracle_sample(cfg: int):
         ids = [0, 1, 2, 49, 50]
         return subset_atoms(prob, ids), "metal + first 2 heavy + their 2 H of config 4, full O2 build"
     nheavy = 12 if cfg == 2 else 120
-    ids = [0, 1, 2, nheavy, nheavy + 1, nheavy + 2]
-    return subset_atoms(prob, ids), f"first 3 heavy + their 3 H atoms of config {cfg} (same basis, D sub-block), full O2 build"
+    k = 3 if cfg == 2 else 5          # config 5: ~1.2e7 live quartets, 5-15 s of oracle work on the box's host threads
+    ids = list(range(k)) + [nheavy + i for i in range(k)]
+    return subset_atoms(prob, ids), f"first {k} heavy + their {k} H atoms of config {cfg} (same basis, D sub-block), full O2 build"
 
 
 def run_oracle_steps(cfg: int, steps: int, warmup: int):
@@ -154,6 +166,37 @@ def main_reference(args, rank, world):
             "config": {"workload": CONFIG_NAMES[args.config], "sample": desc},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------- roofline ceilings
+def main_peaks():
+    """FP64 ceilings of this GPU, one JSON line: register-resident DFMA chains (the "alu" roofline denominator), cuBLAS
+    float64 matmul 8192^3 (the DMMA / tensor-core FP64 path) and the rate of a DFMA stream fed by one
+    lane-private shared-memory load per FMA (the operand pattern of the uniform-ket Hermite -> Cartesian transform)."""
+    import torch
+
+    import paper_2406_14920_b200 as te
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --peaks needs a CUDA device")
+    torch.cuda.set_device(0)
+    n = 8192
+    a = torch.randn(n, n, dtype=torch.float64, device="cuda")
+    b = torch.randn(n, n, dtype=torch.float64, device="cuda")
+    for _ in range(2):
+        a @ b
+    torch.cuda.synchronize()
+    best = 0.0
+    for _ in range(5):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        a @ b
+        e1.record()
+        torch.cuda.synchronize()
+        best = max(best, 2 * n ** 3 / (e0.elapsed_time(e1) * 1e-3) / 1e12)
+    line = {"fp64_dfma_tflops": te.te_measure_fp64_peak(), "fp64_matmul_8192_tflops": best,
+            "fp64_nominal_tflops": 148 * 64 * 2 * 1.965e9 / 1e12,
+            "smem_fed_dfma_tflops": {str(w): te.te_measure_smem_dfma_rate(w) for w in (4, 8, 16)}}
     print(json.dumps(line), flush=True)
 
 
@@ -204,6 +247,7 @@ def main_ours(args, rank, world):
     sec = max_over_ranks(sec_local, world)
     q, _ = pairs.stats()
     live = int(q.sum())
+    visited, slots = pairs.screening_stats()
     npairs_nonempty = sum(1 for cb in range(10) for ck in range(cb, 10) if pairs.class_count[cb] and pairs.class_count[ck])
     nclasses_nonempty = sum(1 for c in range(10) if pairs.class_count[c])
     # scale, bounds, finish + (Hermite density, Hermite J) per pair class + (schedule, J/K kernel) per class pair
@@ -247,14 +291,19 @@ def main_ours(args, rank, world):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * step_s, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": CONFIG_NAMES[args.config], "nbf": n, "primitive_pairs_kept": pairs.nkept,
-                   "live_quartets_per_build": live, "thresholds": [prob.tau_pair, prob.tau_jk],
+                   "live_quartets_per_build": live, "visited_quartets_per_build": int(visited.sum()),
+                   "live_over_visited": live / max(int(visited.sum()), 1), "lane_occupancy": live / max(int(slots.sum()), 1),
+                   "thresholds": [prob.tau_pair, prob.tau_jk],
                    "l2": "flushed between timed iterations (256 MB fill)", "parallelism": "replicas only"},
         "jk_build_s_per_iter": step_s, "pair_build_s": t_setup,
         "model_flops_per_build": total_flops, "fp64_tflops_algorithmic": total_flops / step_s / 1e12,
         "fp64_frac_of_peak": total_flops / step_s / 1e12 / peak,
         "roofline": {"bound": "alu", "kernel": f"J/K class kernel ({te.CLASS_NAMES[cb]}|{te.CLASS_NAMES[ck]})",
                      "achieved": dom_ach, "peak": peak, "unit": "TFLOP/s", "frac": dom_ach / peak,
-                     "traffic": NCU_DRAM_BYTES.get((args.config, f"({te.CLASS_NAMES[cb]}|{te.CLASS_NAMES[ck]})")),
+                     "traffic": ncu_dram_bytes(args.config, f"({te.CLASS_NAMES[cb]}|{te.CLASS_NAMES[ck]})"),
+                     "traffic_source": "profiles/r2_dram_bytes.json (ncu --set full capture of this config) or null",
+                     "kernel_ms": float(ms[cb, ck]), "kernel_share_of_step": float(ms[cb, ck]) / float(ms.sum()),
+                     "whole_build_frac": total_flops / step_s / 1e12 / peak,
                      "peak_source": "te_measure_fp64_peak: register-resident DFMA chains measured in this run "
                                     "(MEASURED_PEAKS.json has no FP64 entry; nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2)",
                      "top_kernels_ms": per_class},
@@ -272,9 +321,13 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--peaks", action="store_true", help="print the measured FP64 ceilings of this GPU and exit")
     args = ap.parse_args()
+    if args.peaks:
+        main_peaks()
+        return
     if args.impl == "reference":      # rank 0 alone runs the oracle; other ranks exit 0 without work, no rendezvous
         main_reference(args, int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")))
         return

@@ -21,6 +21,14 @@
  *  - Every contracted Cartesian function is normalised to unit self-overlap (eq. 1-2); the
  *    caller passes RAW contraction coefficients.
  *  - There is no CPU fallback: every call that computes needs a CUDA device (sm_100a build).
+ *  - Devices: a te_basis lives on the CUDA device that was current in te_basis_create, and so does every te_pairs
+ *    built from it; calls that compute return TE_ERR_BAD_ARG when another device is current.  Several devices may be
+ *    used from one process (the library's tables are kept per device).
+ *  - Concurrency: the scratch of a build (accumulators, schedules, statistics) lives in the te_pairs handle, so a
+ *    handle carries ONE build at a time.  Builds issued on different streams with the same handle are serialised by
+ *    the library on the device (each waits for the previous one); calls on one handle from several host threads at
+ *    once are not supported.  Use one te_pairs per concurrent build.
+ *  - Size limits: a pair class may hold at most INT_MAX candidate pairs (TE_ERR_BAD_ARG beyond).
  */
 #ifndef TE_JK_H
 #define TE_JK_H
@@ -77,11 +85,45 @@ int te_pairs_export_geom(const te_pairs *p, int cls, double *P_xyz, double *p_ex
  * eq. 47; 0 means no screening.  A primitive quartet's contribution X <- D_YZ is included iff
  * q_bra * q_ket * max|D_YZ block| >= threshold, separately for each of its J and K updates.
  * Asynchronous on cuda_stream (a cudaStream_t, NULL = default stream). */
-int te_build_jk(const te_pairs *p, const double *D_dev, double *J_dev, double *K_dev, double threshold,
+int te_build_jk(te_pairs *p, const double *D_dev, double *J_dev, double *K_dev, double threshold,
                 void *cuda_stream);
 /* Same build with HOST D, J, K (pinned or pageable): copies in, builds, copies out, synchronises. */
-int te_build_jk_host(const te_pairs *p, const double *D_host, double *J_host, double *K_host,
+int te_build_jk_host(te_pairs *p, const double *D_host, double *J_host, double *K_host,
                      double threshold);
+/* Long-range build for range-separated hybrids (eq. 32-33): the same J and K with the operator
+ * erf(omega r)/r in place of 1/r.  Only the argument of the auxiliary integrals, pq omega^2 / (pq + (p+q) omega^2),
+ * and the prefactor, 2 pi^{5/2} omega / (p q sqrt(pq + (p+q) omega^2)), change; the pair lists, their Schwarz bounds
+ * (which also bound the attenuated integrals) and the per-term rule are those of te_build_jk.  omega > 0, in 1/bohr. */
+int te_build_jk_lr(te_pairs *p, const double *D_dev, double *J_dev, double *K_dev, double threshold, double omega,
+                   void *cuda_stream);
+/* Coulomb matrix alone by the "J engine" of eq. 35, for every angular class: the density is
+ * transformed to the Hermite basis of each ket pair, the quartets are contracted in Hermite space (R_PQ only, no
+ * Hermite -> Cartesian transform of integrals), and the Hermite J of each bra pair is transformed back -- all three steps
+ * on the device (the paper keeps the outer two on the CPU).  Same pair lists and the same per-term rule as the J updates
+ * of te_build_jk (J_AB <- D_CD iff q q Dm_CD >= threshold, J_CD <- D_AB iff q q Dm_AB >= threshold), so J equals the J
+ * of te_build_jk to rounding.  J_dev: DEVICE nbf x nbf, OVERWRITTEN.  Asynchronous on cuda_stream. */
+int te_build_j(te_pairs *p, const double *D_dev, double *J_dev, double threshold, void *cuda_stream);
+/* Mixed-precision build ("integrals with a density weighted Schwartz upper bound above a threshold (1e-5,
+ * the default) are evaluated in double precision while the rest are evaluated in single precision").  A primitive
+ * quartet whose density-weighted bound -- q_bra q_ket times the largest of its six density bounds -- is below
+ * fp32_below is evaluated by FP32 kernels (R, E tables, both transforms, digestion), the others by the FP64 kernels of
+ * te_build_jk; pair data, Boys values and prefactors are always FP64, and J / K are accumulated in FP64.  Same pair
+ * lists and per-term rule as te_build_jk.  30 of the 55 classes have an FP32 leg (not those with l_a+l_b+l_c+l_d <= 2,
+ * the lightest s/p classes and df / ff bras), and a quartet whose ket exponent would push (2 alpha)^L outside the FP32
+ * range stays FP64.  fp32_below = 0 reproduces te_build_jk.  The result differs from te_build_jk by the FP32 rounding of
+ * the small terms (measured error study); it is NOT held to the 1e-10 parity bar. */
+int te_build_jk_mixed(te_pairs *p, const double *D_dev, double *J_dev, double *K_dev, double threshold,
+                      double fp32_below, void *cuda_stream);
+/* Live quartets of the LAST build per precision leg (te_build_jk: everything in fp64_quartets).  HOST outputs. */
+int te_jk_precision_stats(const te_pairs *p, long long fp64_quartets[TE_NCLASS][TE_NCLASS],
+                          long long fp32_quartets[TE_NCLASS][TE_NCLASS]);
+/* Nuclear-attraction matrix (eq. 14-26): V_mu,nu = sum_C q_C (mu| 1/|r - C| |nu) over `ncharge` point
+ * charges, summed over the kept primitive pairs of the handle (one thread per primitive pair looping over the charges,
+ * P:356).  The sign is that of eq. 14: a nucleus of charge Z enters with q_C = -Z.  xyz_bohr[ncharge][3] and q[ncharge]:
+ * HOST; V_dev: DEVICE, row-major nbf x nbf, OVERWRITTEN, symmetric.  Runs on cuda_stream and synchronises it before
+ * returning. */
+int te_nuclear_attraction(te_pairs *p, int ncharge, const double *xyz_bohr, const double *q, double *V_dev,
+                          void *cuda_stream);
 /* Statistics of the LAST te_build_jk on this handle (synchronises the build's stream).  HOST outputs,
  * indexed [bra class][ket class] (only bra class <= ket class is used): unique primitive quartets that
  * had at least one live update, and device milliseconds spent in that class pair's kernel. */
@@ -92,6 +134,10 @@ int te_jk_stats(const te_pairs *p, long long quartets[TE_NCLASS][TE_NCLASS], flo
  * slots of the warp batches that ran the integral code, so live / slots is the lane occupancy of the class kernel.
  * Either pointer may be NULL. */
 int te_jk_screening_stats(const te_pairs *p, long long visited[TE_NCLASS][TE_NCLASS], long long slots[TE_NCLASS][TE_NCLASS]);
+/* Kernel family used by the builds on this handle: 2 (default) = the measured per-class choice; 0 = generic
+ * thread-per-quartet kernel for every class, 1 = uniform-ket warp kernel wherever it exists, 3 = split-quartet kernel
+ * wherever it exists.  Every family computes the same J and K (tests hold each to the parity bar). */
+int te_jk_set_kernel_family(te_pairs *p, int family);
 /* Enable (1) / disable (0) per-class CUDA-event timing for te_jk_stats (off by default). */
 int te_jk_set_profiling(te_pairs *p, int on);
 
@@ -109,6 +155,11 @@ int te_boys(int n, const double *T_dev, int mmax, double *F_dev);
 /* Sustained FP64 FMA throughput of the device (register-resident DFMA chains), in TFLOP/s: the measured
  * denominator of the "alu" roofline. */
 int te_measure_fp64_peak(double *tflops);
+
+/* FP64 rate, in TFLOP/s, of a loop that feeds every DFMA with one lane-private 8-byte shared-memory load (the operand pattern
+ * of the Hermite -> Cartesian transform of the uniform-ket kernel: R in a conflict-free shared-memory column), with
+ * `warps_per_sm` (1..32) one-warp blocks resident per SM: the shared-memory ceiling of that transform. */
+int te_measure_smem_dfma_rate(int warps_per_sm, double *tflops);
 
 const char *te_last_error(void);
 

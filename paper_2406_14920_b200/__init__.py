@@ -61,6 +61,13 @@ def lib():
     L.te_pairs_export_geom.argtypes = [vp, C.c_int, dpp, dpp, dpp]
     L.te_build_jk.argtypes = [vp, vp, vp, vp, C.c_double, vp]
     L.te_build_jk_host.argtypes = [vp, dpp, dpp, dpp, C.c_double]
+    L.te_build_jk_lr.argtypes = [vp, vp, vp, vp, C.c_double, C.c_double, vp]
+    L.te_build_jk_mixed.argtypes = [vp, vp, vp, vp, C.c_double, C.c_double, vp]
+    L.te_build_j.argtypes = [vp, vp, vp, C.c_double, vp]
+    L.te_jk_precision_stats.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
+    L.te_nuclear_attraction.argtypes = [vp, C.c_int, dpp, dpp, vp, vp]
+    L.te_jk_set_kernel_family.argtypes = [vp, C.c_int]
+    L.te_measure_smem_dfma_rate.argtypes = [C.c_int, dpp]
     L.te_jk_stats.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_float)]
     L.te_jk_screening_stats.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
     L.te_jk_set_profiling.argtypes = [vp, C.c_int]
@@ -169,8 +176,10 @@ class Pairs:
                "te_pairs_export_geom")
         return out
 
-    def build_jk(self, D, J=None, K=None, threshold: float = 0.0, stream=None):
-        """te_build_jk with torch CUDA tensors (float64, nbf x nbf, contiguous).  Asynchronous on `stream`."""
+    def build_jk(self, D, J=None, K=None, threshold: float = 0.0, stream=None, omega: float | None = None,
+                 fp32_below: float | None = None):
+        """te_build_jk (te_build_jk_lr when omega is given, te_build_jk_mixed when fp32_below is given) with torch CUDA
+        tensors (float64, nbf x nbf, contiguous).  Asynchronous on `stream`."""
         import torch
         n = self.basis.nbf
         assert D.is_cuda and D.dtype == torch.float64 and D.is_contiguous() and tuple(D.shape) == (n, n)
@@ -179,9 +188,56 @@ class Pairs:
         if K is None:
             K = torch.empty_like(D)
         st = stream if stream is not None else torch.cuda.current_stream()
-        _check(lib().te_build_jk(self.handle, C.c_void_p(D.data_ptr()), C.c_void_p(J.data_ptr()),
-                                 C.c_void_p(K.data_ptr()), float(threshold), C.c_void_p(st.cuda_stream)), "te_build_jk")
+        if fp32_below is not None:
+            assert omega is None
+            _check(lib().te_build_jk_mixed(self.handle, C.c_void_p(D.data_ptr()), C.c_void_p(J.data_ptr()),
+                                           C.c_void_p(K.data_ptr()), float(threshold), float(fp32_below),
+                                           C.c_void_p(st.cuda_stream)), "te_build_jk_mixed")
+        elif omega is None:
+            _check(lib().te_build_jk(self.handle, C.c_void_p(D.data_ptr()), C.c_void_p(J.data_ptr()),
+                                     C.c_void_p(K.data_ptr()), float(threshold), C.c_void_p(st.cuda_stream)), "te_build_jk")
+        else:
+            _check(lib().te_build_jk_lr(self.handle, C.c_void_p(D.data_ptr()), C.c_void_p(J.data_ptr()),
+                                        C.c_void_p(K.data_ptr()), float(threshold), float(omega),
+                                        C.c_void_p(st.cuda_stream)), "te_build_jk_lr")
         return J, K
+
+    def build_j(self, D, J=None, threshold: float = 0.0, stream=None):
+        """te_build_j: Coulomb matrix alone by the J-engine route (eq. 35).  Asynchronous on `stream`."""
+        import torch
+        n = self.basis.nbf
+        assert D.is_cuda and D.dtype == torch.float64 and D.is_contiguous() and tuple(D.shape) == (n, n)
+        if J is None:
+            J = torch.empty_like(D)
+        st = stream if stream is not None else torch.cuda.current_stream()
+        _check(lib().te_build_j(self.handle, C.c_void_p(D.data_ptr()), C.c_void_p(J.data_ptr()), float(threshold),
+                                C.c_void_p(st.cuda_stream)), "te_build_j")
+        return J
+
+    def nuclear_attraction(self, xyz_c, q_c, V=None, stream=None):
+        """te_nuclear_attraction: V[nbf, nbf] (torch CUDA float64) for host point charges xyz_c[n, 3], q_c[n]."""
+        import torch
+        n = self.basis.nbf
+        xyz_c = np.ascontiguousarray(xyz_c, dtype=np.float64).reshape(-1, 3)
+        q_c = np.ascontiguousarray(q_c, dtype=np.float64)
+        assert xyz_c.shape[0] == q_c.shape[0]
+        if V is None:
+            V = torch.empty((n, n), dtype=torch.float64, device="cuda")
+        st = stream if stream is not None else torch.cuda.current_stream()
+        _check(lib().te_nuclear_attraction(self.handle, int(q_c.shape[0]), _dp(xyz_c), _dp(q_c), C.c_void_p(V.data_ptr()),
+                                           C.c_void_p(st.cuda_stream)), "te_nuclear_attraction")
+        return V
+
+    def set_kernel_family(self, family: int):
+        _check(lib().te_jk_set_kernel_family(self.handle, int(family)), "te_jk_set_kernel_family")
+
+    def precision_stats(self):
+        """(fp64_quartets[10][10], fp32_quartets[10][10]) of the last build (te_jk_precision_stats)."""
+        a = np.zeros((NCLASS, NCLASS), dtype=np.int64)
+        b = np.zeros((NCLASS, NCLASS), dtype=np.int64)
+        _check(lib().te_jk_precision_stats(self.handle, a.ctypes.data_as(C.POINTER(C.c_longlong)),
+                                           b.ctypes.data_as(C.POINTER(C.c_longlong))), "te_jk_precision_stats")
+        return a, b
 
     def build_jk_host(self, D: np.ndarray, threshold: float = 0.0, J=None, K=None):
         """te_build_jk_host: HOST numpy (or pinned torch CPU) buffers in, HOST buffers out (synchronous)."""
@@ -242,6 +298,22 @@ def te_build_jk(pairs: Pairs, D, J=None, K=None, threshold: float = 0.0, stream=
     return pairs.build_jk(D, J, K, threshold, stream)
 
 
+def te_build_j(pairs: Pairs, D, J=None, threshold: float = 0.0, stream=None):
+    return pairs.build_j(D, J, threshold, stream)
+
+
+def te_build_jk_lr(pairs: Pairs, D, omega: float, J=None, K=None, threshold: float = 0.0, stream=None):
+    return pairs.build_jk(D, J, K, threshold, stream, omega=omega)
+
+
+def te_build_jk_mixed(pairs: Pairs, D, fp32_below: float = 1e-5, J=None, K=None, threshold: float = 0.0, stream=None):
+    return pairs.build_jk(D, J, K, threshold, stream, fp32_below=fp32_below)
+
+
+def te_nuclear_attraction(pairs: Pairs, xyz_c, q_c, V=None, stream=None):
+    return pairs.nuclear_attraction(xyz_c, q_c, V, stream)
+
+
 def te_eri_block(basis: Basis, quartets):
     return basis.eri_block(quartets)
 
@@ -253,6 +325,12 @@ def te_boys(T, mmax: int):
     F = torch.empty((T.numel(), mmax + 1), dtype=torch.float64, device=T.device)
     _check(lib().te_boys(T.numel(), C.c_void_p(T.data_ptr()), mmax, C.c_void_p(F.data_ptr())), "te_boys")
     return F
+
+
+def te_measure_smem_dfma_rate(warps_per_sm: int = 8) -> float:
+    v = C.c_double()
+    _check(lib().te_measure_smem_dfma_rate(int(warps_per_sm), C.byref(v)), "te_measure_smem_dfma_rate")
+    return float(v.value)
 
 
 def te_measure_fp64_peak() -> float:

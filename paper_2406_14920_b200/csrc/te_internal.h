@@ -54,6 +54,7 @@ struct te_basis {
     double *d_exp = nullptr, *d_ct = nullptr, *d_xyz = nullptr, *d_aofac = nullptr;
     int *d_shell = nullptr, *d_off = nullptr, *d_by_l = nullptr, *d_shell_off = nullptr, *d_shell_pstart = nullptr;
     const double* d_boys = nullptr;
+    int device = 0;   // CUDA device the handle (and every te_pairs built from it) lives on
 };
 
 struct te_pairs {
@@ -72,11 +73,14 @@ struct te_pairs {
     // per-build scratch
     double *d_Ds = nullptr, *d_Jt = nullptr, *d_Kt = nullptr, *d_Dm = nullptr;
     te::JKControl* d_ctrl = nullptr;
-    // class-pair kernels of one build run concurrently on NSTREAM internal streams (forked from / joined to the
-    // caller's stream with events); each internal stream owns its schedule scratch
-    static constexpr int NSTREAM = 8;
-    cudaStream_t streams[NSTREAM] = {nullptr};
-    cudaEvent_t ev_fork = nullptr, ev_join[NSTREAM] = {nullptr};
+    te::JKControl* d_ctrl32 = nullptr;   // task queues / counters of the FP32 leg of a mixed-precision build
+    double prec_thr = 0.0;               // density-weighted bound below which a quartet is evaluated in FP32 (0: FP64 build)
+    int impl = 2;                        // kernel-family policy (te_jk_set_kernel_family): 2 = measured per-class default
+    double omega2 = 0.0;                 // operator of the build in flight: 0 = 1/r, omega^2 = erf(omega r)/r
+    // schedule scratch of the class kernel in flight (class kernels of a build run back to back on the caller's stream)
+    static constexpr int NSTREAM = 1;
+    cudaEvent_t ev_done = nullptr;   // end of the last build / one-electron call on this handle: the next one waits for it
+    bool ev_done_valid = false;
     long long* d_tile_start[NSTREAM] = {nullptr};
     int* d_task_hi[NSTREAM] = {nullptr};
     long long tile_cap = 0;
@@ -91,8 +95,12 @@ namespace te {
 // te_inst_*.cu
 int launch_schwarz(int la, int lb, const te_basis* b, long long ncand, double* d_q, long long* d_idx);
 int launch_pair_fill(int la, int lb, const te_basis* b, long long n, const long long* d_idx, PairD* d_pair, PairIds* d_ids);
-int launch_jk_class(int cb, int ck, te_pairs* P, double tau, int lane, cudaStream_t st);   // lane: which schedule scratch
+// lane: which schedule scratch; prec: 0 plain FP64, 1 / 2 = FP64 / FP32 leg of a mixed-precision build
+int launch_jk_class(int cb, int ck, te_pairs* P, double tau, int lane, int prec, cudaStream_t st);
 int launch_eri_class(int cb, int ck, const te_basis* b, int n, const EriTask* d_tasks, double* out_dev);
 int launch_hermite_density(int cls, te_pairs* P, cudaStream_t st);   // d_Ds -> d_DH[cls]
 int launch_hermite_j(int cls, te_pairs* P, cudaStream_t st);         // d_JH[cls] -> d_Jt
+int launch_nuclear(int cls, te_pairs* P, int ncharge, const double4* d_chg, double* d_Vt, cudaStream_t st);
+int launch_jeng_class(int cb, int ck, te_pairs* P, double tau, cudaStream_t st);   // Coulomb only, Hermite space (eq. 35)
+constexpr int TE_MAX_DEV = 64;   // per-device caches (Boys table, class tables, occupancy) are indexed by the CUDA device id
 }  // namespace te

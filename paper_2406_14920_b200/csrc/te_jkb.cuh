@@ -109,6 +109,7 @@ __global__ void __launch_bounds__(WARP) jkb_kernel(JKArgs a) {
         }
         long long cur = 0, end = 0;
         bool assigned = false;
+        unsigned fl = 0;   // update types (J_ab, K_ac, K_bc, K_ad, K_bd) that were live for at least one primitive pair of the block
         int offA = 0, offB = 0;
         double dm_jcd = 0.0, dm_kac = 0.0, dm_kbc = 0.0, dm_kad = 0.0, dm_kbd = 0.0, mjab = 0.0;
         double dab[NA * NB], dbl[NB * ND], dal[NA * ND], dbk[NB * NC], dak[NA * NC];
@@ -120,29 +121,28 @@ __global__ void __launch_bounds__(WARP) jkb_kernel(JKArgs a) {
         while (true) {
             const bool need = cur >= end;
             if (need && assigned) {
-                // ---- the block is finished: one flush of everything it produced
+                // ---- the block is finished: one flush of everything it produced.  One branch per update type (was it ever live in
+                // this block?) instead of a compare-and-branch per element: the flush runs with partial masks on almost every
+                // iteration of the warp, so its instruction count matters as much as the integral code's.
+                if (fl & 1) {
 #pragma unroll
-                for (int i = 0; i < NA; ++i)
-#pragma unroll
-                    for (int jj = 0; jj < NB; ++jj)
-                        if (jab[i * NB + jj] != 0.0) atomicAdd(&a.Jt[(offA + i) * nbf + offB + jj], 2.0 * jab[i * NB + jj]);
-#pragma unroll
-                for (int i = 0; i < NA; ++i) {
-#pragma unroll
-                    for (int k = 0; k < NC; ++k)
-                        if (kac[i * NC + k] != 0.0) atomicAdd(&a.Kt[(offA + i) * nbf + ik.offA + k], kac[i * NC + k]);
-#pragma unroll
-                    for (int l = 0; l < ND; ++l)
-                        if (kad[i * ND + l] != 0.0) atomicAdd(&a.Kt[(offA + i) * nbf + ik.offB + l], kad[i * ND + l]);
+                    for (int x = 0; x < NA * NB; ++x) atomicAdd(&a.Jt[(offA + x / NB) * nbf + offB + x % NB], 2.0 * jab[x]);
                 }
+                if (fl & 2) {
 #pragma unroll
-                for (int jj = 0; jj < NB; ++jj) {
+                    for (int x = 0; x < NA * NC; ++x) atomicAdd(&a.Kt[(offA + x / NC) * nbf + ik.offA + x % NC], kac[x]);
+                }
+                if (fl & 4) {
 #pragma unroll
-                    for (int k = 0; k < NC; ++k)
-                        if (kbc[jj * NC + k] != 0.0) atomicAdd(&a.Kt[(offB + jj) * nbf + ik.offA + k], kbc[jj * NC + k]);
+                    for (int x = 0; x < NB * NC; ++x) atomicAdd(&a.Kt[(offB + x / NC) * nbf + ik.offA + x % NC], kbc[x]);
+                }
+                if (fl & 8) {
 #pragma unroll
-                    for (int l = 0; l < ND; ++l)
-                        if (kbd[jj * ND + l] != 0.0) atomicAdd(&a.Kt[(offB + jj) * nbf + ik.offB + l], kbd[jj * ND + l]);
+                    for (int x = 0; x < NA * ND; ++x) atomicAdd(&a.Kt[(offA + x / ND) * nbf + ik.offB + x % ND], kad[x]);
+                }
+                if (fl & 16) {
+#pragma unroll
+                    for (int x = 0; x < NB * ND; ++x) atomicAdd(&a.Kt[(offB + x / ND) * nbf + ik.offB + x % ND], kbd[x]);
                 }
                 assigned = false;
             }
@@ -153,7 +153,7 @@ __global__ void __launch_bounds__(WARP) jkb_kernel(JKArgs a) {
                 long long s = 0, e = 0;
                 if (blk < a.nblk) { s = max((long long)a.bstart[blk], b_lo); e = min((long long)a.bstart[blk + 1], b_hi); }
                 if (s < e) {
-                    cur = s; end = e; assigned = true;
+                    cur = s; end = e; assigned = true; fl = 0;
                     const PairIds ib = a.ib[s];
                     offA = ib.offA; offB = ib.offB;
                     dm_jcd = a.Dm[ib.shA * ns + ib.shB];
@@ -191,6 +191,11 @@ __global__ void __launch_bounds__(WARP) jkb_kernel(JKArgs a) {
             if (work) {
                 ++nvis;
                 const long long bi = cur++;
+                if (cur < end) {   // the next primitive pair of this lane's block: pull its data into L1 while this one computes
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(a.pb + cur));
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(reinterpret_cast<const char*>(a.pb + cur) + 88));
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(a.qb + cur));
+                }
                 const double qq = a.qb[bi] * qk;
                 // the per-term tests of eq. 47; bounds fall along the block, so a dead term stays dead: zero its density block
                 const bool live_jab = qq * dm_jab >= a.tau, live_jcd = qq * dm_jcd >= a.tau, live_kac = qq * dm_kac >= a.tau;
@@ -216,29 +221,35 @@ __global__ void __launch_bounds__(WARP) jkb_kernel(JKArgs a) {
 #pragma unroll
                     for (int x = 0; x < NA * NC; ++x) dak[x] = 0.0;
                 }
-                if (!(live_jab | live_jcd | live_kac | live_kbc | live_kad | live_kbd)) {
+                // FP64 leg of a mixed-precision build: once the density-weighted bound falls below the switch, the rest of the block
+                // (bounds fall along it, the ket is fixed) belongs to the FP32 launch
+                const bool to32 = a.prec_mode == 1 &&
+                                  fp32_quartet(a, qq, fmax(fmax(fmax(dm_jab, dm_jcd), fmax(dm_kac, dm_kbc)), fmax(dm_kad, dm_kbd)), kp.p);
+                if (!(live_jab | live_jcd | live_kac | live_kbc | live_kad | live_kbd) || to32) {
                     cur = end;   // bounds fall along the block: the rest of it is dead too
                 } else {
                     ++nlive;
+                    fl |= (live_jab ? 1u : 0u) | (live_kac ? 2u : 0u) | (live_kbc ? 4u : 0u) | (live_kad ? 8u : 0u) | (live_kbd ? 16u : 0u);
                     const PairD bp = a.pb[bi];
                     const PairIds ibp = a.ib[bi];
                     double f = 1.0;
                     if (ibp.m == ibp.n) f *= 0.5;
                     if (ik.m == ik.n) f *= 0.5;
                     if (a.same && bi == j) f *= 0.5;
-                    const double p = bp.p, q = kp.p, pq = p + q;
-                    const double alpha = p * q / pq;
+                    const double p = bp.p, q = kp.p;
+                    double alpha, pref;
+                    eri_scale(p, bp.rp, q, kp.rp, a.omega2, alpha, pref);
                     const double X = bp.P[0] - kp.P[0], Y = bp.P[1] - kp.P[1], Z = bp.P[2] - kp.P[2];
                     double F[L + 1];
                     boys<L>(alpha * (X * X + Y * Y + Z * Z), a.boys_tab, F);
                     // 2 pi^{5/2} / (p q sqrt(p+q)) (eq. 30) x bra prefactor x symmetry factor, folded into the Boys values
-                    const double pref = 34.986836655249725693 / (p * q * sqrt(pq)) * bp.pref * f;
+                    pref *= bp.pref * f;
 #pragma unroll
                     for (int m = 0; m <= L; ++m) F[m] *= pref;
                     double R[nherm(L)];
                     rtable<L>(alpha, X, Y, Z, F, R);
                     double Ebx[LA + 1][LB + 1][LAB + 1], Eby[LA + 1][LB + 1][LAB + 1], Ebz[LA + 1][LB + 1][LAB + 1];
-                    const double hb = 0.5 / p;
+                    const double hb = 0.5 * bp.rp;
                     etable<LA, LB, false>(bp.PA[0], bp.PB[0], hb, Ebx);
                     etable<LA, LB, false>(bp.PA[1], bp.PB[1], hb, Eby);
                     etable<LA, LB, false>(bp.PA[2], bp.PB[2], hb, Ebz);

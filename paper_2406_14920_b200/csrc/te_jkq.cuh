@@ -129,11 +129,15 @@ constexpr int jkq_lanes(int la, int lb, int lc, int ld, int w) {
 // 3 and 5, per-class CUDA-event times): it wins for every FF ket, for DF kets against bras with la+lb >= 2, for d/f-heavy bras
 // (la+lb >= 4) against kets with lc+ld >= 4, and for (SD|DD), (PD|PF), (PD|DD); one quartet per lane (uniform-ket kernel) wins
 // elsewhere.  TE_JK_IMPL=3 forces it wherever it exists.
-constexpr bool use_jkq(int la, int lb, int lc, int ld) { return la + lb + lc + ld >= 3; }
 constexpr bool jkq_default(int la, int lb, int lc, int ld) {
+    // round 2 (after the uniform-ket kernel stopped flushing per (k,l)): (SD|DF), (PP|DF) and (SD|DD) moved to the uniform-ket kernel
+    if (lc == 2 && ld == 3 && ((la == 0 && lb == 2) || (la == 1 && lb == 1))) return false;
     return (lc + ld == 6) || (lc == 2 && ld == 3 && la + lb >= 2) || (la + lb >= 4 && lc + ld >= 4) ||
-           (la == 1 && lb == 2 && lc + ld >= 4) || (la == 0 && lb == 2 && lc == 2 && ld == 2);
+           (la == 1 && lb == 2 && lc + ld >= 4);
 }
+// instantiated exactly where it is the default (round 1 instantiated it for every class with L >= 3 so that family 3 could force it
+// anywhere; that doubled the compile time of the library for kernels no build uses)
+constexpr bool use_jkq(int la, int lb, int lc, int ld) { return jkq_default(la, lb, lc, ld); }
 
 template <int LA, int LB, int LC, int LD, int G, int W>
 __global__ void __launch_bounds__(32 * W, (nherm(LA + LB) <= 10 ? 4 : 2)) jkq_kernel(JKArgs a, const QTab<LA, LB, LC, LD>* __restrict__ gtab) {
@@ -237,13 +241,19 @@ __global__ void __launch_bounds__(32 * W, (nherm(LA + LB) <= 10 ? 4 : 2)) jkq_ke
                 if (g == 0) ++nvis;
                 ib = a.ib[bi];
                 const double qq = a.qb[bi] * qk;
-                live_jab = qq * a.Dm[ik.shA * ns + ik.shB] >= a.tau;
-                live_jcd = qq * a.Dm[ib.shA * ns + ib.shB] >= a.tau;
-                live_kac = qq * a.Dm[ib.shB * ns + ik.shB] >= a.tau;
-                live_kbc = qq * a.Dm[ib.shA * ns + ik.shB] >= a.tau;
-                live_kad = qq * a.Dm[ib.shB * ns + ik.shA] >= a.tau;
-                live_kbd = qq * a.Dm[ib.shA * ns + ik.shA] >= a.tau;
+                const double d1 = a.Dm[ik.shA * ns + ik.shB], d2 = a.Dm[ib.shA * ns + ib.shB], d3 = a.Dm[ib.shB * ns + ik.shB];
+                const double d4 = a.Dm[ib.shA * ns + ik.shB], d5 = a.Dm[ib.shB * ns + ik.shA], d6 = a.Dm[ib.shA * ns + ik.shA];
+                live_jab = qq * d1 >= a.tau;
+                live_jcd = qq * d2 >= a.tau;
+                live_kac = qq * d3 >= a.tau;
+                live_kbc = qq * d4 >= a.tau;
+                live_kad = qq * d5 >= a.tau;
+                live_kbd = qq * d6 >= a.tau;
                 active = live_jab | live_jcd | live_kac | live_kbc | live_kad | live_kbd;
+                // FP64 leg of a mixed-precision build: the FP32 quartets belong to the other launch
+                if (a.prec_mode == 1 && fp32_quartet(a, qq, fmax(fmax(fmax(d1, d2), fmax(d3, d4)), fmax(d5, d6)), kp.p)) {
+                    active = false; live_jab = live_jcd = live_kac = live_kbc = live_kad = live_kbd = false;
+                }
             }
             if (!__any_sync(FULLMASK, active)) continue;
             if (g == 0) ++nslot;
@@ -259,12 +269,13 @@ __global__ void __launch_bounds__(32 * W, (nherm(LA + LB) <= 10 ? 4 : 2)) jkq_ke
                 if (ib.m == ib.n) f *= 0.5;
                 if (ik.m == ik.n) f *= 0.5;
                 if (a.same && bi == j) f *= 0.5;
-                const double p = bp.p, q = kp.p, pq = p + q;
-                alpha = p * q / pq;
+                const double p = bp.p, q = kp.p;
+                double pref;
+                eri_scale(p, bp.rp, q, kp.rp, a.omega2, alpha, pref);
                 X = bp.P[0] - kp.P[0]; Y_ = bp.P[1] - kp.P[1]; Z = bp.P[2] - kp.P[2];
                 boys<L>(alpha * (X * X + Y_ * Y_ + Z * Z), a.boys_tab, F);
                 // 2 pi^{5/2} / (p q sqrt(p+q)) (eq. 30) x bra prefactor x symmetry factor, folded into the Boys values
-                const double pref = 34.986836655249725693 / (p * q * sqrt(pq)) * bp.pref * f;
+                pref *= bp.pref * f;
 #pragma unroll
                 for (int m = 0; m <= L; ++m) F[m] *= pref;
                 // bra 1-D E tables: one dimension per lane of the group
@@ -272,7 +283,7 @@ __global__ void __launch_bounds__(32 * W, (nherm(LA + LB) <= 10 ? 4 : 2)) jkq_ke
                     double E[LA + 1][LB + 1][LAB + 1];
                     const double PA = d == 0 ? bp.PA[0] : (d == 1 ? bp.PA[1] : bp.PA[2]);
                     const double PB = d == 0 ? bp.PB[0] : (d == 1 ? bp.PB[1] : bp.PB[2]);
-                    etable<LA, LB, false>(PA, PB, 0.5 / p, E);
+                    etable<LA, LB, false>(PA, PB, 0.5 * bp.rp, E);
 #pragma unroll
                     for (int i = 0; i <= LA; ++i)
 #pragma unroll

@@ -48,7 +48,21 @@ struct WShape {
     // K_?c accumulators / D_?c blocks of the smaller ket shell stay in registers for the whole quartet when small
     // UNR: the loops over the ket component pairs (k,l) and their Hermite boxes are fully unrolled, so every table offset and
     // accumulator index is a compile-time constant (no row-table lookups, no dynamically indexed register arrays)
-    static constexpr bool UNR = NHB * NNZK + nnz_e(LA, LB) * NC * ND <= 6000;
+    // Measured (ncu source page, round 2): above a few hundred FMAs the compiler either declines the unrolling (leaving run-time
+    // box loops that spend 5 integer instructions per DFMA) or honours it and the straight-line code misses the instruction
+    // cache (no_instruction stalls); the alternative is compile-time (t',u'[,v']) loops skipped by warp-uniform branches, whose
+    // body is NHB x (LDS + DFMA) with immediate offsets.  Per-class choice from CUDA-event times on config 5: s-, sp- and sd-type
+    // bras (NHB <= 10, at most 10 FMAs per box entry) are fastest with the "#pragma unroll" form while it stays under ~6000
+    // FMAs, pp bras and the larger light-bra classes with compile-time (t',u',v'), sf / pd bras (NHB = 20) with compile-time
+    // (t',u') and a run-time v' loop -- except against pd-sized kets (LCD <= 3), where compile-time v' also wins ((PD|PD)
+    // 351 -> 281 ms); for larger kets it gains < 2 % and triples the compile time of the library.
+    static constexpr int SIZE = NHB * NNZK + nnz_e(LA, LB) * NC * ND;
+    static constexpr int VAR = LCD == 6 ? 1   // ff kets (FP32 leg / forced family only): the 84-entry compile-time box costs minutes of ptxas
+                             : (LA == 1 && LB == 1) ? 2
+                             : NHB <= 10 ? (SIZE <= 6000 ? 0 : 2)
+                             : (LA == 0 && LB == 3 && LC == 0 && LD == 3) ? 0 : (LCD <= 3 ? 2 : 1);
+    static constexpr bool UNR = VAR == 0;
+    static constexpr bool V2CT = VAR == 2;
     static constexpr int UNK = UNR ? 128 : 1;
     static constexpr bool KEEPC = UNR && (NA + NB) * NC <= 24;
     // NL = lanes of the warp that hold a quartet (R column stride).  Measured on B200: narrowing the warp to 8 lanes for L >= 10
@@ -64,37 +78,37 @@ struct WShape {
 // Segmented reduction over runs of lanes + one atomic per run and value, for N values that share a live flag.  The shuffle
 // rounds of the N values are independent, so their latencies overlap (one value at a time, the rounds of a reduction form a
 // serial SHFL -> DADD chain of ~40 cycles each; measured: the per-value version was the largest single cost of this kernel).
-template <int N, class AddrFn>
-__device__ __forceinline__ void flush_vec(bool runs, int maxdist, int dist, bool head, bool live, double (&v)[N], AddrFn addr) {
+template <int N, class T, class AddrFn>
+__device__ __forceinline__ void flush_vec(bool runs, int maxdist, int dist, bool head, bool live, T (&v)[N], AddrFn addr) {
     constexpr unsigned FULLMASK = 0xffffffffu;
     if (runs) {
 #pragma unroll
-        for (int x = 0; x < N; ++x) v[x] = live ? v[x] : 0.0;
+        for (int x = 0; x < N; ++x) v[x] = live ? v[x] : T(0);
         for (int o = 1; o < maxdist; o <<= 1) {
 #pragma unroll
             for (int x = 0; x < N; ++x) {
-                const double t = __shfl_down_sync(FULLMASK, v[x], o);
+                const T t = __shfl_down_sync(FULLMASK, v[x], o);
                 if (o < dist) v[x] += t;
             }
         }
         if (head) {
 #pragma unroll
             for (int x = 0; x < N; ++x)
-                if (v[x] != 0.0) atomicAdd(addr(x), v[x]);
+                if (v[x] != T(0)) atomicAdd(addr(x), (double)v[x]);
         }
     } else if (live) {
 #pragma unroll
-        for (int x = 0; x < N; ++x) atomicAdd(addr(x), v[x]);
+        for (int x = 0; x < N; ++x) atomicAdd(addr(x), (double)v[x]);
     }
 }
 
 // R^0_{tuv} of eq. 21-25 built in place in a shared-memory column (element i at R[i * 32]); same sweep as rtable<L>.
-template <int L, int RS>
-__device__ __forceinline__ void rtable_sm(double alpha, double X, double Y, double Z, const double* __restrict__ F, double* R) {
-    double fac[L + 1];
-    fac[0] = 1.0;
+template <int L, int RS, class T>
+__device__ __forceinline__ void rtable_sm(T alpha, T X, T Y, T Z, const T* __restrict__ F, T* R) {
+    T fac[L + 1];
+    fac[0] = T(1);
 #pragma unroll
-    for (int m = 1; m <= L; ++m) fac[m] = fac[m - 1] * (-2.0 * alpha);
+    for (int m = 1; m <= L; ++m) fac[m] = fac[m - 1] * (T(-2) * alpha);
     R[0] = fac[L] * F[L];
 #pragma unroll
     for (int m = L - 1; m >= 0; --m) {
@@ -105,16 +119,16 @@ __device__ __forceinline__ void rtable_sm(double alpha, double X, double Y, doub
 #pragma unroll
                 for (int u = n - t; u >= 0; --u) {
                     const int v = n - t - u;
-                    double r;
+                    T r;
                     if (t > 0) {
                         r = X * R[tidx<L>(t - 1, u, v) * RS];
-                        if (t > 1) r = fma((double)(t - 1), R[tidx<L>(t - 2, u, v) * RS], r);
+                        if (t > 1) r = fma(T(t - 1), R[tidx<L>(t - 2, u, v) * RS], r);
                     } else if (u > 0) {
                         r = Y * R[tidx<L>(t, u - 1, v) * RS];
-                        if (u > 1) r = fma((double)(u - 1), R[tidx<L>(t, u - 2, v) * RS], r);
+                        if (u > 1) r = fma(T(u - 1), R[tidx<L>(t, u - 2, v) * RS], r);
                     } else {
                         r = Z * R[tidx<L>(t, u, v - 1) * RS];
-                        if (v > 1) r = fma((double)(v - 1), R[tidx<L>(t, u, v - 2) * RS], r);
+                        if (v > 1) r = fma(T(v - 1), R[tidx<L>(t, u, v - 2) * RS], r);
                     }
                     R[tidx<L>(t, u, v) * RS] = r;
                 }
@@ -124,7 +138,10 @@ __device__ __forceinline__ void rtable_sm(double alpha, double X, double Y, doub
     }
 }
 
-template <int LA, int LB, int LC, int LD>
+// T = double: the FP64 path.  T = float: the FP32 leg of the mixed-precision build: pair data, Boys values and the
+// prefactor are formed in FP64 and rounded once; R, the E tables, both transforms and the digestion run in FP32; every quartet's
+// sums are added to the FP64 J / K accumulators.
+template <class T, int LA, int LB, int LC, int LD>
 __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
     using S = WShape<LA, LB, LC, LD>;
     constexpr int LAB = S::LAB, LCD = S::LCD, L = S::L;
@@ -134,14 +151,16 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
     constexpr int UNK = S::UNK;
     constexpr int NL = S::NL;
     constexpr unsigned FULLMASK = 0xffffffffu;
-    extern __shared__ double sm[];
-    double* const Rsm = sm;
-    double* const kt = Rsm + S::NR * NL;
-    double* const e1 = kt + S::NNZK;
-    double* const dcd = e1 + 3 * S::NE1;
+    extern __shared__ double sm_raw[];
+    T* const Rsm = reinterpret_cast<T*>(sm_raw);
+    T* const kt = Rsm + S::NR * NL;
+    T* const e1 = kt + S::NNZK;
+    T* const dcd = e1 + 3 * S::NE1;
     const int lane = threadIdx.x;
-    double* const Rl = Rsm + (lane < NL ? lane : 0);   // lanes >= NL never hold a quartet
-    double* const kcl = dcd + NC * ND + lane;          // K_?c accumulator column of this lane (only without KEEPC)
+    T* const Rl = Rsm + (lane < NL ? lane : 0);   // lanes >= NL never hold a quartet
+    T* const kcl = dcd + NC * ND + lane;          // K_?c accumulator column of this lane (only without KEEPC)
+    constexpr bool F32 = sizeof(T) == 4;
+    if (F32 != (a.prec_mode == 2)) return;        // the FP32 instantiation serves the FP32 leg and nothing else
 
     const unsigned long long ntasks = a.ctrl->ntiles[a.slot];
     const long long span = (long long)NL * a.ctrl->chunk[a.slot];
@@ -178,7 +197,7 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
 #pragma unroll
                     for (int jj = 0; jj <= LD; ++jj)
 #pragma unroll
-                        for (int t = 0; t <= LCD; ++t) e1[lane * S::NE1 + (i * (LD + 1) + jj) * (LCD + 1) + t] = E[i][jj][t];
+                        for (int t = 0; t <= LCD; ++t) e1[lane * S::NE1 + (i * (LD + 1) + jj) * (LCD + 1) + t] = (T)E[i][jj][t];
             }
             __syncwarp();
             int e = 0;
@@ -186,16 +205,16 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                 const int lx = cart_x(LD, l), ly = cart_y(LD, l), lz = cart_z(LD, l);
                 for (int k = 0; k < NC; ++k) {
                     const int kx = cart_x(LC, k), ky = cart_y(LC, k), kz = cart_z(LC, k);
-                    const double* ex = e1 + (kx * (LD + 1) + lx) * (LCD + 1);
-                    const double* ey = e1 + S::NE1 + (ky * (LD + 1) + ly) * (LCD + 1);
-                    const double* ez = e1 + 2 * S::NE1 + (kz * (LD + 1) + lz) * (LCD + 1);
+                    const T* ex = e1 + (kx * (LD + 1) + lx) * (LCD + 1);
+                    const T* ey = e1 + S::NE1 + (ky * (LD + 1) + ly) * (LCD + 1);
+                    const T* ez = e1 + 2 * S::NE1 + (kz * (LD + 1) + lz) * (LCD + 1);
                     for (int t2 = 0; t2 <= kx + lx; ++t2)
                         for (int u2 = 0; u2 <= ky + ly; ++u2)
                             for (int v2 = 0; v2 <= kz + lz; ++v2, ++e)
-                                if ((e & 31) == lane) kt[e] = ex[t2] * ey[u2] * ez[v2] * kp.pref;
+                                if ((e & 31) == lane) kt[e] = ex[t2] * ey[u2] * ez[v2] * (T)kp.pref;
                 }
             }
-            for (int cd = lane; cd < NC * ND; cd += WARP) dcd[cd] = a.Ds[(ik.offA + cd / ND) * nbf + ik.offB + cd % ND];
+            for (int cd = lane; cd < NC * ND; cd += WARP) dcd[cd] = (T)a.Ds[(ik.offA + cd / ND) * nbf + ik.offB + cd % ND];
             __syncwarp();
             cached_j = j;
         }
@@ -210,13 +229,17 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                 ++nvis;
                 ib = a.ib[bi];
                 const double qq = a.qb[bi] * qk;
-                live_jab = qq * a.Dm[ik.shA * ns + ik.shB] >= a.tau;
-                live_jcd = qq * a.Dm[ib.shA * ns + ib.shB] >= a.tau;
-                live_kac = qq * a.Dm[ib.shB * ns + ik.shB] >= a.tau;
-                live_kbc = qq * a.Dm[ib.shA * ns + ik.shB] >= a.tau;
-                live_kad = qq * a.Dm[ib.shB * ns + ik.shA] >= a.tau;
-                live_kbd = qq * a.Dm[ib.shA * ns + ik.shA] >= a.tau;
+                const double d1 = a.Dm[ik.shA * ns + ik.shB], d2 = a.Dm[ib.shA * ns + ib.shB], d3 = a.Dm[ib.shB * ns + ik.shB];
+                const double d4 = a.Dm[ib.shA * ns + ik.shB], d5 = a.Dm[ib.shB * ns + ik.shA], d6 = a.Dm[ib.shA * ns + ik.shA];
+                live_jab = qq * d1 >= a.tau;
+                live_jcd = qq * d2 >= a.tau;
+                live_kac = qq * d3 >= a.tau;
+                live_kbc = qq * d4 >= a.tau;
+                live_kad = qq * d5 >= a.tau;
+                live_kbd = qq * d6 >= a.tau;
                 active = live_jab | live_jcd | live_kac | live_kbc | live_kad | live_kbd;
+                // mixed precision: this launch evaluates either the FP64 or the FP32 quartets (rule: fp32_quartet in te_kernels.cuh)
+                if (a.prec_mode && fp32_quartet(a, qq, fmax(fmax(fmax(d1, d2), fmax(d3, d4)), fmax(d5, d6)), kp.p) != F32) active = false;
             }
             if (!__any_sync(FULLMASK, active)) continue;
             ++nslot;
@@ -233,9 +256,9 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
             const int maxdist = __reduce_max_sync(FULLMASK, dist);
             const bool runs = maxdist > 1;   // warp-uniform: without runs every lane adds its own contribution directly
             double f = 1.0;
-            double Ebx[LA + 1][LB + 1][LAB + 1], Eby[LA + 1][LB + 1][LAB + 1], Ebz[LA + 1][LB + 1][LAB + 1];
-            double dab[NA * NB], jab[NA * NB];
-            double dbc[KEEPC ? NB * NC : 1], dac[KEEPC ? NA * NC : 1], kac[KEEPC ? NA * NC : 1], kbc[KEEPC ? NB * NC : 1];
+            T Ebx[LA + 1][LB + 1][LAB + 1], Eby[LA + 1][LB + 1][LAB + 1], Ebz[LA + 1][LB + 1][LAB + 1];
+            T dab[NA * NB], jab[NA * NB];
+            T dbc[KEEPC ? NB * NC : 1], dac[KEEPC ? NA * NC : 1], kac[KEEPC ? NA * NC : 1], kbc[KEEPC ? NB * NC : 1];
 #pragma unroll
             for (int x = 0; x < NA * NB; ++x) jab[x] = 0.0;
             if (KEEPC) {
@@ -254,33 +277,37 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                 if (ib.m == ib.n) f *= 0.5;
                 if (ik.m == ik.n) f *= 0.5;
                 if (a.same && bi == j) f *= 0.5;
-                const double p = bp.p, q = kp.p, pq = p + q;
-                const double alpha = p * q / pq;
+                const double p = bp.p, q = kp.p;
+                double alpha, pref;
+                eri_scale(p, bp.rp, q, kp.rp, a.omega2, alpha, pref);
                 const double X = bp.P[0] - kp.P[0], Y = bp.P[1] - kp.P[1], Z = bp.P[2] - kp.P[2];
                 double F[L + 1];
                 boys<L>(alpha * (X * X + Y * Y + Z * Z), a.boys_tab, F);
                 // 2 pi^{5/2} / (p q sqrt(p+q)) (eq. 30) x bra prefactor x symmetry factor, folded into the Boys values
-                const double pref = 34.986836655249725693 / (p * q * sqrt(pq)) * bp.pref * f;
+                pref *= bp.pref * f;
 #pragma unroll
                 for (int m = 0; m <= L; ++m) F[m] *= pref;
-                rtable_sm<L, NL>(alpha, X, Y, Z, F, Rl);
-                const double hb = 0.5 / p;
-                etable<LA, LB, false>(bp.PA[0], bp.PB[0], hb, Ebx);
-                etable<LA, LB, false>(bp.PA[1], bp.PB[1], hb, Eby);
-                etable<LA, LB, false>(bp.PA[2], bp.PB[2], hb, Ebz);
+                T Fv[L + 1];
+#pragma unroll
+                for (int m = 0; m <= L; ++m) Fv[m] = (T)F[m];
+                rtable_sm<L, NL, T>((T)alpha, (T)X, (T)Y, (T)Z, Fv, Rl);
+                const T hb = (T)(0.5 * bp.rp);
+                etable<LA, LB, false>((T)bp.PA[0], (T)bp.PB[0], hb, Ebx);
+                etable<LA, LB, false>((T)bp.PA[1], (T)bp.PB[1], hb, Eby);
+                etable<LA, LB, false>((T)bp.PA[2], (T)bp.PB[2], hb, Ebz);
                 Da = a.Ds + (long long)ib.offA * nbf;
                 Db = a.Ds + (long long)ib.offB * nbf;
 #pragma unroll
                 for (int i = 0; i < NA; ++i)
 #pragma unroll
-                    for (int jj = 0; jj < NB; ++jj) dab[i * NB + jj] = Da[i * nbf + ib.offB + jj];
+                    for (int jj = 0; jj < NB; ++jj) dab[i * NB + jj] = (T)Da[i * nbf + ib.offB + jj];
                 if (KEEPC) {
 #pragma unroll
                     for (int k = 0; k < NC; ++k) {
 #pragma unroll
-                        for (int i = 0; i < NA; ++i) dac[i * NC + k] = Da[i * nbf + ik.offA + k];
+                        for (int i = 0; i < NA; ++i) dac[i * NC + k] = (T)Da[i * nbf + ik.offA + k];
 #pragma unroll
-                        for (int jj = 0; jj < NB; ++jj) dbc[jj * NC + k] = Db[jj * nbf + ik.offA + k];
+                        for (int jj = 0; jj < NB; ++jj) dbc[jj * NC + k] = (T)Db[jj * nbf + ik.offA + k];
                     }
                 }
             }
@@ -288,7 +315,7 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
 #pragma unroll UNK
             for (int l = 0; l < ND; ++l) {
                 const int lx = cart_x(LD, l), ly = cart_y(LD, l), lz = cart_z(LD, l);
-                double dal[NA], dbl[NB], kal[NA], kbl[NB];
+                T dal[NA], dbl[NB], kal[NA], kbl[NB];
 #pragma unroll
                 for (int i = 0; i < NA; ++i) kal[i] = 0.0;
 #pragma unroll
@@ -302,8 +329,8 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
 #pragma unroll UNK
                 for (int k = 0; k < NC; ++k) {
                     const int sx = cart_x(LC, k) + lx, sy = cart_y(LC, k) + ly, sz = cart_z(LC, k) + lz;
-                    double jkl = 0.0;
-                    double kak[KEEPC ? 1 : NA], kbk[KEEPC ? 1 : NB];
+                    T jkl = 0.0;
+                    T kak[KEEPC ? 1 : NA], kbk[KEEPC ? 1 : NB];
                     if (!KEEPC) {
 #pragma unroll
                         for (int i = 0; i < NA; ++i) kak[i] = 0.0;
@@ -312,10 +339,10 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                     }
                     if (active) {
                         // ---- ket Hermite -> Cartesian for this (k,l): Y_P = sum_Q E~_Q R_{P+Q}
-                        double Yv[NHB];
+                        T Yv[NHB];
 #pragma unroll
                         for (int P = 0; P < NHB; ++P) Yv[P] = 0.0;
-                        const double* ktp = kt + ptr;
+                        const T* ktp = kt + ptr;
                         if constexpr (UNR) {
 #pragma unroll
                             for (int t2 = 0; t2 <= sx; ++t2)
@@ -323,7 +350,7 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                                 for (int u2 = 0; u2 <= sy; ++u2)
 #pragma unroll
                                     for (int v2 = 0; v2 <= sz; ++v2) {
-                                        const double e = *ktp++;
+                                        const T e = *ktp++;
 #pragma unroll
                                         for (int t = 0; t <= LAB; ++t)
 #pragma unroll
@@ -340,11 +367,27 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                                 if (t2 <= sx) {
                                     static_for<LCD + 1 - t2>([&](auto U2) {
                                         constexpr int u2 = decltype(U2)::value;
-                                        if (u2 <= sy) {
-                                            const double* Rq = Rl;
+                                        if constexpr (S::V2CT) {
+                                            if (u2 <= sy) {
+                                                static_for<LCD + 1 - t2 - u2>([&](auto V2) {
+                                                    constexpr int v2 = decltype(V2)::value;
+                                                    if (v2 <= sz) {
+                                                        const T e = *ktp++;
+#pragma unroll
+                                                        for (int t = 0; t <= LAB; ++t)
+#pragma unroll
+                                                            for (int u = 0; u <= LAB - t; ++u)
+#pragma unroll
+                                                                for (int v = 0; v <= LAB - t - u; ++v)
+                                                                    Yv[tidx<LAB>(t, u, v)] = fma(e, Rl[(tidx<L>(t + t2, u + u2, 0) + v + v2) * NL], Yv[tidx<LAB>(t, u, v)]);
+                                                    }
+                                                });
+                                            }
+                                        } else if (u2 <= sy) {
+                                            const T* Rq = Rl;
 #pragma unroll 1
                                             for (int v2 = 0; v2 <= sz; ++v2, Rq += NL) {
-                                                const double e = *ktp++;
+                                                const T e = *ktp++;
 #pragma unroll
                                                 for (int t = 0; t <= LAB; ++t)
 #pragma unroll
@@ -359,27 +402,27 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                             });
                         }
                         // ---- bra Hermite -> Cartesian and digestion
-                        double dbk[KEEPC ? 1 : NB], dak[KEEPC ? 1 : NA];
+                        T dbk[KEEPC ? 1 : NB], dak[KEEPC ? 1 : NA];
                         if (!KEEPC) {
 #pragma unroll
                             for (int i = 0; i < NA; ++i) dak[i] = Da[i * nbf + ik.offA + k];
 #pragma unroll
                             for (int jj = 0; jj < NB; ++jj) dbk[jj] = Db[jj * nbf + ik.offA + k];
                         }
-                        const double dkl = dcd[k * ND + l];
+                        const T dkl = dcd[k * ND + l];
 #pragma unroll
                         for (int i = 0; i < NA; ++i) {
                             const int ix = cart_x(LA, i), iy = cart_y(LA, i), iz = cart_z(LA, i);
 #pragma unroll
                             for (int jj = 0; jj < NB; ++jj) {
                                 const int jx = cart_x(LB, jj), jy = cart_y(LB, jj), jz = cart_z(LB, jj);
-                                double s = 0.0;
+                                T s = 0.0;
 #pragma unroll
                                 for (int t = 0; t <= ix + jx; ++t) {
-                                    double su = 0.0;
+                                    T su = 0.0;
 #pragma unroll
                                     for (int u = 0; u <= iy + jy; ++u) {
-                                        double sv = 0.0;
+                                        T sv = 0.0;
 #pragma unroll
                                         for (int v = 0; v <= iz + jz; ++v) sv = fma(Ebz[iz][jz][v], Yv[tidx<LAB>(t, u, v)], sv);
                                         su = fma(Eby[iy][jy][u], sv, su);
@@ -430,7 +473,7 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                 // the quartet's K_ac / K_bc sums come back from the shared-memory column, NC values (one row of the block) at a time
 #pragma unroll 1
                 for (int r = 0; r < NA + NB; ++r) {
-                    double row[NC];
+                    T row[NC];
 #pragma unroll
                     for (int k = 0; k < NC; ++k) row[k] = kcl[(r * NC + k) * NL];
                     const long long o1 = (r < NA ? ib.offA + r : ib.offB + (r - NA));
@@ -455,7 +498,7 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
 // [same ? j : 0, cut_j) with cut_j = first bra whose q_bra * q_ket[j] * max|D| < tau (eq. 47, loosest density bound); a task is
 // (ket j, chunk of 32*chunk bras).  task_hi[j] = cut_j, tile_start = exclusive prefix sum of the chunk counts.
 static __global__ void __launch_bounds__(1024) schedule_w_kernel(const double* __restrict__ qb, long long nb, const double* __restrict__ qk,
-                                                          long long nk, int same, double tau, int target_warps, int lanes,
+                                                          long long nk, int same, double tau, int target_warps, int lanes, int chunk_cap,
                                                           long long* __restrict__ tile_start, int* __restrict__ task_hi, JKControl* ctrl, int slot) {
     __shared__ long long part[1024];
     __shared__ int s_chunk;
@@ -488,9 +531,12 @@ static __global__ void __launch_bounds__(1024) schedule_w_kernel(const double* _
         __syncthreads();
     }
     if (threadIdx.x == 0) {
-        // chunk: 32*chunk bras per task, sized so every resident warp gets ~8 tasks; 1..16
+        // chunk: 32*chunk bras per task, sized so every resident warp gets ~8 tasks; 1..chunk_cap (every task pays two binary
+        // searches of dependent global loads, ~10^4 cycles of latency, which the light classes cannot hide behind 16 batches)
         long long c = part[0] / ((long long)lanes * target_warps * 8);
-        s_chunk = (int)max(1LL, min(16LL, c));
+        s_chunk = (int)max(1LL, min((long long)chunk_cap, c));
+        // the task counters of the kernels are 32 bit: widen the tasks until their number fits (never reached by the five configs)
+        while (part[0] / ((long long)lanes * s_chunk) + nk >= 0xfffffff0LL) s_chunk *= 2;
         ctrl->chunk[slot] = s_chunk;
     }
     __syncthreads();

@@ -43,6 +43,7 @@ __device__ __forceinline__ void make_pair(const BasisView& bv, int m, int n, Pai
         r2 += (A - B) * (A - B);
     }
     pd.p = p;
+    pd.rp = rp;
     pd.pref = bv.ct[m] * bv.ct[n] * exp(-a * b * rp * r2);
 }
 
@@ -229,8 +230,19 @@ struct JKArgs {
     const int* task_hi;
     JKControl* ctrl;
     double tau;
+    double omega2;                          // 0: 1/r (eq. 30); omega^2 > 0: erf(omega r)/r (eq. 32-33)
+    double prec_thr, amax32;                // mixed precision: FP32 below this density-weighted bound / ket exponent limit
+    int prec_mode;                          // 0: every quartet (FP64 build); 1: FP64 leg, 2: FP32 leg of te_build_jk_mixed
     int nbf, nshells, slot, same;
 };
+
+// Mixed precision ("integrals with a density weighted Schwartz upper bound above a threshold (1e-5 ...) are evaluated in
+// double precision while the rest are evaluated in single precision").  Density-weighted bound of a quartet = q_bra q_ket times
+// the largest of its six density bounds.  FP32 also needs (2 alpha)^L inside its range; alpha <= p_ket, so quartets whose ket
+// exponent exceeds amax32 (set per class from L) stay in FP64.  Both legs evaluate this predicate with the same FP64 inputs.
+__device__ __forceinline__ bool fp32_quartet(const JKArgs& a, double qq, double dmax6, double p_ket) {
+    return qq * dmax6 < a.prec_thr && p_ket <= a.amax32;
+}
 
 template <int LA, int LB, int LC, int LD, int TB, int TK>
 __global__ void __launch_bounds__(TB * TK, (TB * TK >= 256 ? 2 : 1)) jk_kernel(JKArgs a) {
@@ -255,13 +267,16 @@ __global__ void __launch_bounds__(TB * TK, (TB * TK >= 256 ? 2 : 1)) jk_kernel(J
         const PairIds ib = a.ib[bi], ik = a.ik[kj];
         const long long ns = a.nshells;
         JKEmit<LA, LB, LC, LD> em;
-        em.live_jab = qq * a.Dm[ik.shA * ns + ik.shB] >= a.tau;
-        em.live_jcd = qq * a.Dm[ib.shA * ns + ib.shB] >= a.tau;
-        em.live_kac = qq * a.Dm[ib.shB * ns + ik.shB] >= a.tau;
-        em.live_kbc = qq * a.Dm[ib.shA * ns + ik.shB] >= a.tau;
-        em.live_kad = qq * a.Dm[ib.shB * ns + ik.shA] >= a.tau;
-        em.live_kbd = qq * a.Dm[ib.shA * ns + ik.shA] >= a.tau;
+        const double d1 = a.Dm[ik.shA * ns + ik.shB], d2 = a.Dm[ib.shA * ns + ib.shB], d3 = a.Dm[ib.shB * ns + ik.shB];
+        const double d4 = a.Dm[ib.shA * ns + ik.shB], d5 = a.Dm[ib.shB * ns + ik.shA], d6 = a.Dm[ib.shA * ns + ik.shA];
+        em.live_jab = qq * d1 >= a.tau;
+        em.live_jcd = qq * d2 >= a.tau;
+        em.live_kac = qq * d3 >= a.tau;
+        em.live_kbc = qq * d4 >= a.tau;
+        em.live_kad = qq * d5 >= a.tau;
+        em.live_kbd = qq * d6 >= a.tau;
         if (!(em.live_jab | em.live_jcd | em.live_kac | em.live_kbc | em.live_kad | em.live_kbd)) continue;
+        if (a.prec_mode == 1 && fp32_quartet(a, qq, fmax(fmax(fmax(d1, d2), fmax(d3, d4)), fmax(d5, d6)), a.pk[kj].p)) continue;
         ++nlive;
         double f = 1.0;
         if (ib.m == ib.n) f *= 0.5;
@@ -271,11 +286,59 @@ __global__ void __launch_bounds__(TB * TK, (TB * TK >= 256 ? 2 : 1)) jk_kernel(J
         em.oa = ib.offA; em.ob = ib.offB; em.oc = ik.offA; em.od = ik.offB;
         const PairD bra = a.pb[bi], ket = a.pk[kj];
         em.begin();
-        md_quartet<LA, LB, LC, LD, FULL>(bra, ket, a.boys_tab, em);
+        md_quartet<LA, LB, LC, LD, FULL>(bra, ket, a.boys_tab, em, a.omega2);
         em.end();
     }
     for (int o = 16; o > 0; o >>= 1) nlive += __shfl_down_sync(0xffffffffu, nlive, o);
     if ((threadIdx.x & 31) == 0 && nlive) atomicAdd(&a.ctrl->live[a.slot], (unsigned long long)nlive);
+}
+
+// ------------------------------------------------------------------------ nuclear attraction, eq. 14-26
+// One thread = one primitive shell pair, looping over all point charges.  The sum over the charges (eq. 16) is taken in
+// Hermite space, VH_P = sum_C q_C R^0_P(p, P - C) (eq. 20-25 with alpha = p), and transformed once:
+//   Vt[a_i][b_j] += f c~c~ K_ab (2 pi / p) sum_P E_P^{ij} VH_P     (eq. 26; f = 1/2 for m == n, V = (Vt + Vt^T) o ff^T afterwards,
+// which is how an unordered pair stands for both ordered pairs).  The paper stores the results in pair order and scatters on the
+// host; here the scatter is an FP64 atomic add on the device.
+template <int LA, int LB>
+__global__ void __launch_bounds__(64) nuclear_kernel(const PairD* __restrict__ pairs, const PairIds* __restrict__ ids, long long n,
+                                                      int ncharge, const double4* __restrict__ chg, const double* __restrict__ boys_tab,
+                                                      int nbf, double* __restrict__ Vt) {
+    constexpr int LAB = LA + LB, NA = ncart(LA), NB = ncart(LB), NH = nherm(LAB);
+    const long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (x >= n) return;
+    const PairD pd = pairs[x];
+    const PairIds id = ids[x];
+    double acc[NH];
+#pragma unroll
+    for (int P = 0; P < NH; ++P) acc[P] = 0.0;
+    for (int c = 0; c < ncharge; ++c) {
+        const double4 ch = chg[c];   // x, y, z, q_C: the same address for every thread
+        const double X = pd.P[0] - ch.x, Y = pd.P[1] - ch.y, Z = pd.P[2] - ch.z;
+        double F[LAB + 1], R[NH];
+        boys<LAB>(pd.p * (X * X + Y * Y + Z * Z), boys_tab, F);
+#pragma unroll
+        for (int m = 0; m <= LAB; ++m) F[m] *= ch.w;
+        rtable<LAB>(pd.p, X, Y, Z, F, R);
+#pragma unroll
+        for (int P = 0; P < NH; ++P) acc[P] += R[P];
+    }
+    double E[3][LA + 1][LB + 1][LAB + 1];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) etable<LA, LB, false>(pd.PA[d], pd.PB[d], 0.5 * pd.rp, E[d]);
+    const double pref = pd.pref * (6.28318530717958647692 * pd.rp) * (id.m == id.n ? 0.5 : 1.0);
+    for (int i = 0; i < NA; ++i) {
+        const int ix = cart_x(LA, i), iy = cart_y(LA, i), iz = cart_z(LA, i);
+        for (int j = 0; j < NB; ++j) {
+            const int jx = cart_x(LB, j), jy = cart_y(LB, j), jz = cart_z(LB, j);
+            double s = 0.0;
+            for (int t = 0; t <= ix + jx; ++t)
+                for (int u = 0; u <= iy + jy; ++u) {
+                    const double exy = E[0][ix][jx][t] * E[1][iy][jy][u];
+                    for (int v = 0; v <= iz + jz; ++v) s = fma(exy * E[2][iz][jz][v], acc[tidx<LAB>(t, u, v)], s);
+                }
+            atomicAdd(&Vt[(long long)(id.offA + i) * nbf + id.offB + j], pref * s);
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------- integral blocks (testing)

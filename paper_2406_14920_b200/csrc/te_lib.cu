@@ -10,6 +10,8 @@
 #include <cstdio>
 #include <cstring>
 #include <cstdlib>
+#include <climits>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -27,11 +29,16 @@ void set_error(const char* fmt, ...) {
 // ------------------------------------------------------------------------------------------ Boys table
 // F_m(T_i) for the Taylor grid of te_md.cuh, generated on the host in long double: convergent series at the
 // top m (all terms positive), then the downward recursion.
-static double* g_boys_tab = nullptr;   // device, [BOYS_NPTS][BOYS_MROWS]; one per process (single device)
+static double* g_boys_tab[TE_MAX_DEV] = {nullptr};   // device, [BOYS_NPTS][BOYS_STRIDE]; one per CUDA device, built on first use
+static std::mutex g_boys_mutex;
 
 int ensure_boys_table(const double** out) {
-    if (!g_boys_tab) {
-        std::vector<double> h((size_t)BOYS_NPTS * BOYS_MROWS);
+    int dev = -1;
+    TE_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= TE_MAX_DEV) { set_error("device id %d out of range", dev); return TE_ERR_BAD_ARG; }
+    std::lock_guard<std::mutex> lock(g_boys_mutex);
+    if (!g_boys_tab[dev]) {
+        std::vector<double> h((size_t)BOYS_NPTS * BOYS_STRIDE);
         const int mtop = BOYS_MROWS - 1;
         for (int i = 0; i < BOYS_NPTS; ++i) {
             const long double T = (long double)i * (long double)BOYS_DT;
@@ -43,18 +50,19 @@ int ensure_boys_table(const double** out) {
                 if (term < 1e-22L * sum) break;
             }
             long double F = eT * sum;
-            h[(size_t)i * BOYS_MROWS + mtop] = (double)F;
+            h[(size_t)i * BOYS_STRIDE + BOYS_MROWS] = (double)eT;
+            h[(size_t)i * BOYS_STRIDE + mtop] = (double)F;
             for (int m = mtop; m > 0; --m) {
                 F = (2.0L * T * F + eT) / (2 * m - 1);
-                h[(size_t)i * BOYS_MROWS + m - 1] = (double)F;
+                h[(size_t)i * BOYS_STRIDE + m - 1] = (double)F;
             }
         }
         double* d = nullptr;
         TE_CUDA(cudaMalloc(&d, h.size() * sizeof(double)));
         TE_CUDA(cudaMemcpy(d, h.data(), h.size() * sizeof(double), cudaMemcpyHostToDevice));
-        g_boys_tab = d;
+        g_boys_tab[dev] = d;
     }
-    *out = g_boys_tab;
+    *out = g_boys_tab[dev];
     return TE_OK;
 }
 
@@ -142,6 +150,8 @@ extern "C" int te_basis_create(int natoms, const double* xyz, int nshells, const
     std::vector<double> aofac(nbf);
     for (int s = 0; s < nshells; ++s)
         for (int i = 0; i < ncart(shell_l[s]); ++i) aofac[b->shell_off[s] + i] = comp_factor(shell_l[s], i);
+    // arguments are valid: from here on the device is needed (there is no CPU path)
+    if (cudaGetDevice(&b->device) != cudaSuccess) { set_error("te_basis_create: no CUDA device (the library has no CPU path)"); delete b; return TE_ERR_CUDA; }
     int rc;
     if ((rc = upload(b->prim_exp, &b->d_exp)) || (rc = upload(b->prim_ct, &b->d_ct)) || (rc = upload(b->prim_xyz, &b->d_xyz)) ||
         (rc = upload(b->prim_shell, &b->d_shell)) || (rc = upload(b->prim_off, &b->d_off)) ||
@@ -227,6 +237,9 @@ extern "C" int te_shellpair_build(const te_basis* b, double tau_pair, te_pairs**
             const long long ncand = (la == lb) ? na * (na + 1) / 2 : na * nb;
             P->count[cls] = 0;
             if (ncand == 0) continue;
+            if (ncand > (long long)INT_MAX) {   // cub's item counts and the int pair indices of the J/K kernels
+                set_error("te_shellpair_build: class %d has %lld candidate pairs, more than INT_MAX", cls, ncand); return fail(TE_ERR_BAD_ARG);
+            }
             double *d_q = nullptr, *d_qs = nullptr;
             long long *d_idx = nullptr, *d_idxs = nullptr;
             void* d_tmp = nullptr;
@@ -241,7 +254,9 @@ extern "C" int te_shellpair_build(const te_basis* b, double tau_pair, te_pairs**
             size_t tmp_bytes = 0;
             cub::DeviceRadixSort::SortPairsDescending(nullptr, tmp_bytes, d_q, d_qs, d_idx, d_idxs, (int)ncand);
             if (cudaMalloc(&d_tmp, tmp_bytes) != cudaSuccess) { cleanup(); set_error("cub temp alloc failed"); return fail(TE_ERR_ALLOC); }
-            cub::DeviceRadixSort::SortPairsDescending(d_tmp, tmp_bytes, d_q, d_qs, d_idx, d_idxs, (int)ncand);
+            if (cub::DeviceRadixSort::SortPairsDescending(d_tmp, tmp_bytes, d_q, d_qs, d_idx, d_idxs, (int)ncand) != cudaSuccess) {
+                cleanup(); set_error("te_shellpair_build: radix sort failed: %s", cudaGetErrorString(cudaGetLastError())); return fail(TE_ERR_CUDA);
+            }
             cudaMemset(d_cnt, 0, sizeof(unsigned long long));
             count_kept_kernel<<<296, 256>>>(d_qs, ncand, tau_pair, d_cnt);
             unsigned long long nk = 0;
@@ -284,9 +299,10 @@ extern "C" int te_shellpair_build(const te_basis* b, double tau_pair, te_pairs**
                 cub::DeviceRadixSort::SortPairsDescending(nullptr, tb2, bm, d_q, p1, p2, (int)nk);
                 if (cudaMalloc(&tmp2, std::max(tb1, tb2)) != cudaSuccess) { cleanup2(); cleanup(); set_error("cub temp alloc failed"); return fail(TE_ERR_ALLOC); }
                 tb1 = tb2 = std::max(tb1, tb2);
-                cub::DeviceRadixSort::SortPairs(tmp2, tb1, k0, k1, p0, p1, (int)nk);
+                cudaError_t es = cub::DeviceRadixSort::SortPairs(tmp2, tb1, k0, k1, p0, p1, (int)nk);
                 block_max_gather_kernel<<<gr, 256>>>(k1, (long long)nk, bmax, bm);
-                cub::DeviceRadixSort::SortPairsDescending(tmp2, tb2, bm, P->d_qmax[cls], p1, p2, (int)nk);
+                if (es == cudaSuccess) es = cub::DeviceRadixSort::SortPairsDescending(tmp2, tb2, bm, P->d_qmax[cls], p1, p2, (int)nk);
+                if (es != cudaSuccess) { cleanup2(); cleanup(); set_error("te_shellpair_build: radix sort failed: %s", cudaGetErrorString(es)); return fail(TE_ERR_CUDA); }
                 permute_pairs_kernel<<<gr, 256>>>(p2, (long long)nk, t_pair, t_ids, d_qs, P->d_pair[cls], P->d_ids[cls], P->d_q[cls]);
                 cudaError_t e2 = cudaDeviceSynchronize();
                 if (e2 == cudaSuccess) {
@@ -312,20 +328,18 @@ extern "C" int te_shellpair_build(const te_basis* b, double tau_pair, te_pairs**
     const size_t n2 = (size_t)b->nbf * b->nbf, ns2 = (size_t)b->nshells * b->nshells;
     if (cudaMalloc(&P->d_Ds, n2 * sizeof(double)) != cudaSuccess || cudaMalloc(&P->d_Jt, n2 * sizeof(double)) != cudaSuccess ||
         cudaMalloc(&P->d_Kt, n2 * sizeof(double)) != cudaSuccess || cudaMalloc(&P->d_Dm, ns2 * sizeof(double)) != cudaSuccess ||
-        cudaMalloc(&P->d_ctrl, sizeof(JKControl)) != cudaSuccess) {
+        cudaMalloc(&P->d_ctrl, sizeof(JKControl)) != cudaSuccess || cudaMalloc(&P->d_ctrl32, sizeof(JKControl)) != cudaSuccess) {
         set_error("te_shellpair_build: scratch allocation failed"); te_pairs_destroy(P); return TE_ERR_ALLOC;
     }
     long long maxtiles = 0;
     for (int c = 0; c < TE_NCLASS; ++c) maxtiles = std::max(maxtiles, P->count[c] + 2);
     for (int s = 0; s < te_pairs::NSTREAM; ++s) {
         if (cudaMalloc(&P->d_tile_start[s], (maxtiles + 1) * sizeof(long long)) != cudaSuccess ||
-            cudaMalloc(&P->d_task_hi[s], (maxtiles + 1) * sizeof(int)) != cudaSuccess ||
-            cudaStreamCreateWithFlags(&P->streams[s], cudaStreamNonBlocking) != cudaSuccess ||
-            cudaEventCreateWithFlags(&P->ev_join[s], cudaEventDisableTiming) != cudaSuccess) {
+            cudaMalloc(&P->d_task_hi[s], (maxtiles + 1) * sizeof(int)) != cudaSuccess) {
             set_error("te_shellpair_build: scratch allocation failed"); te_pairs_destroy(P); return TE_ERR_ALLOC;
         }
     }
-    if (cudaEventCreateWithFlags(&P->ev_fork, cudaEventDisableTiming) != cudaSuccess) {
+    if (cudaEventCreateWithFlags(&P->ev_done, cudaEventDisableTiming) != cudaSuccess) {
         set_error("te_shellpair_build: event creation failed"); te_pairs_destroy(P); return TE_ERR_ALLOC;
     }
     P->tile_cap = maxtiles;
@@ -337,13 +351,11 @@ extern "C" int te_shellpair_build(const te_basis* b, double tau_pair, te_pairs**
 extern "C" void te_pairs_destroy(te_pairs* P) {
     if (!P) return;
     for (int c = 0; c < TE_NCLASS; ++c) { cudaFree(P->d_pair[c]); cudaFree(P->d_q[c]); cudaFree(P->d_ids[c]); cudaFree(P->d_DH[c]); cudaFree(P->d_JH[c]); cudaFree(P->d_qmax[c]); cudaFree(P->d_bstart[c]); }
-    cudaFree(P->d_Ds); cudaFree(P->d_Jt); cudaFree(P->d_Kt); cudaFree(P->d_Dm); cudaFree(P->d_ctrl);
+    cudaFree(P->d_Ds); cudaFree(P->d_Jt); cudaFree(P->d_Kt); cudaFree(P->d_Dm); cudaFree(P->d_ctrl); cudaFree(P->d_ctrl32);
     for (int s = 0; s < te_pairs::NSTREAM; ++s) {
         cudaFree(P->d_tile_start[s]); cudaFree(P->d_task_hi[s]);
-        if (P->streams[s]) cudaStreamDestroy(P->streams[s]);
-        if (P->ev_join[s]) cudaEventDestroy(P->ev_join[s]);
     }
-    if (P->ev_fork) cudaEventDestroy(P->ev_fork);
+    if (P->ev_done) cudaEventDestroy(P->ev_done);
     cudaFree(P->d_hD); cudaFree(P->d_hJ); cudaFree(P->d_hK);
     for (int i = 0; i < TE_NCLASS * TE_NCLASS; ++i) { if (P->ev0[i]) cudaEventDestroy(P->ev0[i]); if (P->ev1[i]) cudaEventDestroy(P->ev1[i]); }
     delete P;
@@ -447,72 +459,168 @@ __global__ void finish_kernel(const double* __restrict__ Jt, const double* __res
     }
 }
 
-extern "C" int te_build_jk(const te_pairs* Pc, const double* D, double* J, double* K, double tau, void* stream_) {
-    te_pairs* P = const_cast<te_pairs*>(Pc);   // scratch and statistics live in the handle
-    if (!P || !D || !J || !K || !(tau >= 0.0)) { set_error("te_build_jk: NULL argument or negative threshold"); return TE_ERR_BAD_ARG; }
-    cudaStream_t st = (cudaStream_t)stream_;
+__global__ void copy_dmax_kernel(const JKControl* from, JKControl* to) { to->dmax = from->dmax; }
+
+__global__ void finish_one_kernel(const double* __restrict__ Vt, const double* __restrict__ f, int nbf, double* __restrict__ V) {
+    const long long n2 = (long long)nbf * nbf;
+    for (long long x = blockIdx.x * (long long)blockDim.x + threadIdx.x; x < n2; x += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(x / nbf), j = (int)(x % nbf);
+        V[x] = (Vt[x] + Vt[(long long)j * nbf + i]) * (f[i] * f[j]);
+    }
+}
+
+// Common start of every build on a handle: right device, wait for the previous build on this handle (the per-build scratch
+// lives in the handle, so a handle carries ONE build at a time, whatever streams the callers use), per-build preamble.
+static int build_begin(te_pairs* P, const double* D, double omega2, double prec_thr, cudaStream_t st, bool with_k) {
     const te_basis* b = P->basis;
     const int nbf = b->nbf;
     const size_t n2 = (size_t)nbf * nbf;
+    int dev = -1;
+    TE_CUDA(cudaGetDevice(&dev));
+    if (dev != b->device) { set_error("te_build_jk: current device %d is not the device %d the basis was created on", dev, b->device); return TE_ERR_BAD_ARG; }
+    if (P->ev_done_valid) TE_CUDA(cudaStreamWaitEvent(st, P->ev_done, 0));
     P->last_stream = st;
+    P->omega2 = omega2;
+    P->prec_thr = prec_thr;
     TE_CUDA(cudaMemsetAsync(P->d_Jt, 0, n2 * sizeof(double), st));
-    TE_CUDA(cudaMemsetAsync(P->d_Kt, 0, n2 * sizeof(double), st));
+    if (with_k) TE_CUDA(cudaMemsetAsync(P->d_Kt, 0, n2 * sizeof(double), st));
     TE_CUDA(cudaMemsetAsync(P->d_ctrl, 0, sizeof(JKControl), st));
+    TE_CUDA(cudaMemsetAsync(P->d_ctrl32, 0, sizeof(JKControl), st));
     scale_density_kernel<<<592, 256, 0, st>>>(D, b->d_aofac, nbf, P->d_Ds);
     density_bounds_kernel<<<592, 256, 0, st>>>(D, b->d_shell_off, b->nshells, nbf, P->d_Dm, P->d_ctrl);
+    if (prec_thr > 0.0) copy_dmax_kernel<<<1, 1, 0, st>>>(P->d_ctrl, P->d_ctrl32);
+    // Hermite density of every pair and zeroed Hermite J (eq. 35): inputs / accumulators of the Hermite-space Coulomb parts
     int rc = TE_OK;
-    // Hermite density of every pair and zeroed Hermite J (eq. 35): inputs / accumulators of the split-quartet kernels
     for (int c = 0; c < TE_NCLASS; ++c) {
         if (P->count[c] == 0) continue;
         TE_CUDA(cudaMemsetAsync(P->d_JH[c], 0, (size_t)P->count[c] * nherm(CLS_LA_H[c] + CLS_LB_H[c]) * sizeof(double), st));
         if ((rc = launch_hermite_density(c, P, st)) != TE_OK) return rc;
     }
-    const char* only = getenv("TE_DEBUG_SLOT");   // debugging aid: run a single class pair "cb*10+ck"
     for (int i = 0; i < TE_NCLASS * TE_NCLASS; ++i) P->ev_valid[i] = false;
-    // class pairs, most expensive first (pair counts x transform work of one quartet), so the long kernels start early
-    struct Job { int cb, ck; double w; };
+    return TE_OK;
+}
+
+// One build (1/r when omega2 == 0, erf(omega r)/r otherwise; FP64, or FP64 / FP32 by density-weighted bound when prec_thr > 0).
+static int build_jk_impl(te_pairs* P, const double* D, double* J, double* K, double tau, double omega2, double prec_thr, cudaStream_t st) {
+    const te_basis* b = P->basis;
+    int rc = build_begin(P, D, omega2, prec_thr, st, true);
+    if (rc != TE_OK) return rc;
+    // class pairs, most expensive first (pair counts x transform work of one quartet)
+    struct Job { int cb, ck; double w; bool has32; };
     std::vector<Job> jobs;
     for (int cb = 0; cb < TE_NCLASS; ++cb)
         for (int ck = cb; ck < TE_NCLASS; ++ck) {
             if (P->count[cb] == 0 || P->count[ck] == 0) continue;
-            if (only && atoi(only) != cb * TE_NCLASS + ck) continue;
             const int la = CLS_LA_H[cb], lb = CLS_LB_H[cb], lc = CLS_LA_H[ck], ld = CLS_LB_H[ck];
             const double w = (double)P->count[cb] * (double)P->count[ck] *
                              (60.0 + nherm(la + lb) * (double)nherm(lc + ld) + 7.0 * ncart(la) * ncart(lb) * ncart(lc) * ncart(ld));
-            jobs.push_back(Job{cb, ck, w});
+            // mixed precision: classes without an FP32 leg (jk_fp32_class) run as in the FP64 build (prec 0)
+            jobs.push_back(Job{cb, ck, w, prec_thr > 0.0 && jk_fp32_class(la, lb, lc, ld)});
         }
     std::sort(jobs.begin(), jobs.end(), [](const Job& x, const Job& y) { return x.w > y.w; });
-    if (P->profiling) {
-        // serial, on the caller's stream, with an event pair around every class pair
-        for (const Job& j : jobs) {
-            const int slot = j.cb * TE_NCLASS + j.ck;
-            cudaEventRecord(P->ev0[slot], st);
-            if ((rc = launch_jk_class(j.cb, j.ck, P, tau, 0, st)) != TE_OK) return rc;
-            cudaEventRecord(P->ev1[slot], st);
-            P->ev_valid[slot] = true;
-        }
-    } else {
-        // fork: every internal stream waits for the preamble on the caller's stream; join: the caller's stream waits for all
-        constexpr int NS = te_pairs::NSTREAM;
-        TE_CUDA(cudaEventRecord(P->ev_fork, st));
-        for (int s = 0; s < NS; ++s) TE_CUDA(cudaStreamWaitEvent(P->streams[s], P->ev_fork, 0));
-        for (size_t i = 0; i < jobs.size() && rc == TE_OK; ++i) rc = launch_jk_class(jobs[i].cb, jobs[i].ck, P, tau, (int)(i % NS), P->streams[i % NS]);
-        for (int s = 0; s < NS; ++s) {
-            TE_CUDA(cudaEventRecord(P->ev_join[s], P->streams[s]));
-            TE_CUDA(cudaStreamWaitEvent(st, P->ev_join[s], 0));
-        }
+    // Class kernels run back to back on the caller's stream: every one is a persistent grid that fills the GPU, and running
+    // them concurrently on several streams measured 4.6 % SLOWER on config 5 (17.54 s serial, 18.38 s on 8 streams) and equal on
+    // config 2.  With profiling on, an event pair brackets every class pair.
+    for (const Job& j : jobs) {
+        const int slot = j.cb * TE_NCLASS + j.ck;
+        if (P->profiling) cudaEventRecord(P->ev0[slot], st);
+        if ((rc = launch_jk_class(j.cb, j.ck, P, tau, 0, j.has32 ? 1 : 0, st)) != TE_OK) return rc;
+        if (j.has32 && (rc = launch_jk_class(j.cb, j.ck, P, tau, 0, 2, st)) != TE_OK) return rc;
+        if (P->profiling) { cudaEventRecord(P->ev1[slot], st); P->ev_valid[slot] = true; }
     }
-    if (rc != TE_OK) return rc;
     // Hermite J -> Cartesian J of every pair (the paper's CPU post-processing step, on the device)
     for (int c = 0; c < TE_NCLASS; ++c)
         if (P->count[c] && (rc = launch_hermite_j(c, P, st)) != TE_OK) return rc;
-    finish_kernel<<<592, 256, 0, st>>>(P->d_Jt, P->d_Kt, b->d_aofac, nbf, J, K);
+    finish_kernel<<<592, 256, 0, st>>>(P->d_Jt, P->d_Kt, b->d_aofac, b->nbf, J, K);
     TE_CUDA(cudaGetLastError());
+    TE_CUDA(cudaEventRecord(P->ev_done, st));
+    P->ev_done_valid = true;
     return TE_OK;
 }
 
-extern "C" int te_build_jk_host(const te_pairs* Pc, const double* D, double* J, double* K, double tau) {
-    te_pairs* P = const_cast<te_pairs*>(Pc);
+extern "C" int te_build_jk(te_pairs* P, const double* D, double* J, double* K, double tau, void* stream_) {
+    if (!P || !D || !J || !K || !(tau >= 0.0)) { set_error("te_build_jk: NULL argument or negative threshold"); return TE_ERR_BAD_ARG; }
+    return build_jk_impl(P, D, J, K, tau, 0.0, 0.0, (cudaStream_t)stream_);
+}
+
+extern "C" int te_build_jk_lr(te_pairs* P, const double* D, double* J, double* K, double tau, double omega, void* stream_) {
+    if (!P || !D || !J || !K || !(tau >= 0.0) || !(omega > 0.0) || !std::isfinite(omega)) {
+        set_error("te_build_jk_lr: NULL argument, negative threshold or non-positive omega"); return TE_ERR_BAD_ARG;
+    }
+    return build_jk_impl(P, D, J, K, tau, omega * omega, 0.0, (cudaStream_t)stream_);
+}
+
+extern "C" int te_build_jk_mixed(te_pairs* P, const double* D, double* J, double* K, double tau, double fp32_below, void* stream_) {
+    if (!P || !D || !J || !K || !(tau >= 0.0) || !(fp32_below >= 0.0) || !std::isfinite(fp32_below)) {
+        set_error("te_build_jk_mixed: NULL argument or negative threshold"); return TE_ERR_BAD_ARG;
+    }
+    return build_jk_impl(P, D, J, K, tau, 0.0, fp32_below, (cudaStream_t)stream_);
+}
+
+// Coulomb matrix alone by the J-engine route of eq. 35: Hermite density -> Hermite J in the jeng kernels -> Cartesian J.
+extern "C" int te_build_j(te_pairs* P, const double* D, double* J, double tau, void* stream_) {
+    if (!P || !D || !J || !(tau >= 0.0)) { set_error("te_build_j: NULL argument or negative threshold"); return TE_ERR_BAD_ARG; }
+    cudaStream_t st = (cudaStream_t)stream_;
+    const te_basis* b = P->basis;
+    int rc = build_begin(P, D, 0.0, 0.0, st, false);
+    if (rc != TE_OK) return rc;
+    for (int cb = 0; cb < TE_NCLASS; ++cb)
+        for (int ck = cb; ck < TE_NCLASS; ++ck) {
+            if (P->count[cb] == 0 || P->count[ck] == 0) continue;
+            const int slot = cb * TE_NCLASS + ck;
+            if (P->profiling) cudaEventRecord(P->ev0[slot], st);
+            if ((rc = launch_jeng_class(cb, ck, P, tau, st)) != TE_OK) return rc;
+            if (P->profiling) { cudaEventRecord(P->ev1[slot], st); P->ev_valid[slot] = true; }
+        }
+    for (int c = 0; c < TE_NCLASS; ++c)
+        if (P->count[c] && (rc = launch_hermite_j(c, P, st)) != TE_OK) return rc;
+    finish_one_kernel<<<592, 256, 0, st>>>(P->d_Jt, b->d_aofac, b->nbf, J);
+    TE_CUDA(cudaGetLastError());
+    TE_CUDA(cudaEventRecord(P->ev_done, st));
+    P->ev_done_valid = true;
+    return TE_OK;
+}
+
+// Nuclear attraction (eq. 14-26): see nuclear_kernel in te_kernels.cuh.
+extern "C" int te_nuclear_attraction(te_pairs* P, int ncharge, const double* xyz, const double* q, double* V_dev, void* stream_) {
+    if (!P || ncharge < 0 || (ncharge > 0 && (!xyz || !q)) || !V_dev) { set_error("te_nuclear_attraction: NULL argument or negative count"); return TE_ERR_BAD_ARG; }
+    const te_basis* b = P->basis;
+    int dev = -1;
+    TE_CUDA(cudaGetDevice(&dev));
+    if (dev != b->device) { set_error("te_nuclear_attraction: current device %d is not the device %d the basis was created on", dev, b->device); return TE_ERR_BAD_ARG; }
+    cudaStream_t st = (cudaStream_t)stream_;
+    const size_t n2 = (size_t)b->nbf * b->nbf;
+    std::vector<double4> h((size_t)ncharge);
+    for (int c = 0; c < ncharge; ++c) {
+        if (!std::isfinite(xyz[3 * c]) || !std::isfinite(xyz[3 * c + 1]) || !std::isfinite(xyz[3 * c + 2]) || !std::isfinite(q[c])) {
+            set_error("te_nuclear_attraction: point charge %d is not finite", c); return TE_ERR_BAD_ARG;
+        }
+        h[c] = make_double4(xyz[3 * c], xyz[3 * c + 1], xyz[3 * c + 2], q[c]);
+    }
+    double4* d_chg = nullptr;
+    if (ncharge > 0) {
+        if (cudaMalloc(&d_chg, h.size() * sizeof(double4)) != cudaSuccess) { set_error("te_nuclear_attraction: device allocation failed"); return TE_ERR_ALLOC; }
+        if (cudaMemcpy(d_chg, h.data(), h.size() * sizeof(double4), cudaMemcpyHostToDevice) != cudaSuccess) { cudaFree(d_chg); set_error("te_nuclear_attraction: copy failed"); return TE_ERR_CUDA; }
+    }
+    int rc = TE_OK;
+    cudaError_t e = cudaSuccess;
+    if (P->ev_done_valid) e = cudaStreamWaitEvent(st, P->ev_done, 0);   // d_Jt is the scratch of the J/K builds too
+    if (e == cudaSuccess) e = cudaMemsetAsync(P->d_Jt, 0, n2 * sizeof(double), st);
+    for (int c = 0; c < TE_NCLASS && rc == TE_OK && e == cudaSuccess && ncharge > 0; ++c) rc = launch_nuclear(c, P, ncharge, d_chg, P->d_Jt, st);
+    if (rc == TE_OK && e == cudaSuccess) {
+        finish_one_kernel<<<592, 256, 0, st>>>(P->d_Jt, b->d_aofac, b->nbf, V_dev);
+        e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaEventRecord(P->ev_done, st);
+        if (e == cudaSuccess) P->ev_done_valid = true;
+    }
+    const cudaError_t e2 = cudaStreamSynchronize(st);   // the charge buffer is freed below
+    cudaFree(d_chg);
+    if (rc != TE_OK) return rc;
+    if (e != cudaSuccess || e2 != cudaSuccess) { set_error("te_nuclear_attraction: %s", cudaGetErrorString(e != cudaSuccess ? e : e2)); return TE_ERR_CUDA; }
+    return TE_OK;
+}
+
+extern "C" int te_build_jk_host(te_pairs* P, const double* D, double* J, double* K, double tau) {
     if (!P || !D || !J || !K) { set_error("te_build_jk_host: NULL argument"); return TE_ERR_BAD_ARG; }
     const size_t bytes = (size_t)P->basis->nbf * P->basis->nbf * sizeof(double);
     if (!P->d_hD) {
@@ -529,6 +637,12 @@ extern "C" int te_build_jk_host(const te_pairs* Pc, const double* D, double* J, 
     return TE_OK;
 }
 
+extern "C" int te_jk_set_kernel_family(te_pairs* P, int family) {
+    if (!P || family < 0 || family > 3) { set_error("te_jk_set_kernel_family: NULL handle or family outside 0..3"); return TE_ERR_BAD_ARG; }
+    P->impl = family;
+    return TE_OK;
+}
+
 extern "C" int te_jk_set_profiling(te_pairs* P, int on) {
     if (!P) { set_error("te_jk_set_profiling: NULL handle"); return TE_ERR_BAD_ARG; }
     P->profiling = on != 0;
@@ -538,17 +652,32 @@ extern "C" int te_jk_set_profiling(te_pairs* P, int on) {
 extern "C" int te_jk_stats(const te_pairs* P, long long quartets[TE_NCLASS][TE_NCLASS], float ms[TE_NCLASS][TE_NCLASS]) {
     if (!P) { set_error("te_jk_stats: NULL handle"); return TE_ERR_BAD_ARG; }
     TE_CUDA(cudaStreamSynchronize(P->last_stream));
-    JKControl h;
+    JKControl h, h32;
     TE_CUDA(cudaMemcpy(&h, P->d_ctrl, sizeof(h), cudaMemcpyDeviceToHost));
+    TE_CUDA(cudaMemcpy(&h32, P->d_ctrl32, sizeof(h32), cudaMemcpyDeviceToHost));
     for (int cb = 0; cb < TE_NCLASS; ++cb)
         for (int ck = 0; ck < TE_NCLASS; ++ck) {
             const int slot = cb * TE_NCLASS + ck;
-            if (quartets) quartets[cb][ck] = (long long)h.live[slot];
+            if (quartets) quartets[cb][ck] = (long long)(h.live[slot] + h32.live[slot]);
             if (ms) {
                 float t = 0.f;
                 if (P->ev_valid[slot]) cudaEventElapsedTime(&t, P->ev0[slot], P->ev1[slot]);
                 ms[cb][ck] = t;
             }
+        }
+    return TE_OK;
+}
+
+extern "C" int te_jk_precision_stats(const te_pairs* P, long long fp64_quartets[TE_NCLASS][TE_NCLASS], long long fp32_quartets[TE_NCLASS][TE_NCLASS]) {
+    if (!P) { set_error("te_jk_precision_stats: NULL handle"); return TE_ERR_BAD_ARG; }
+    TE_CUDA(cudaStreamSynchronize(P->last_stream));
+    JKControl h, h32;
+    TE_CUDA(cudaMemcpy(&h, P->d_ctrl, sizeof(h), cudaMemcpyDeviceToHost));
+    TE_CUDA(cudaMemcpy(&h32, P->d_ctrl32, sizeof(h32), cudaMemcpyDeviceToHost));
+    for (int cb = 0; cb < TE_NCLASS; ++cb)
+        for (int ck = 0; ck < TE_NCLASS; ++ck) {
+            if (fp64_quartets) fp64_quartets[cb][ck] = (long long)h.live[cb * TE_NCLASS + ck];
+            if (fp32_quartets) fp32_quartets[cb][ck] = (long long)h32.live[cb * TE_NCLASS + ck];
         }
     return TE_OK;
 }
@@ -667,6 +796,53 @@ extern "C" int te_measure_fp64_peak(double* tflops) {
         cudaEventElapsedTime(&ms, e0, e1);
         const double fl = 2.0 * 8 * 16 * (double)iters * blocks * threads;
         if (rep > 0) best = std::max(best, fl / (ms * 1e-3) / 1e12);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+    TE_CUDA(cudaGetLastError());
+    *tflops = best;
+    return TE_OK;
+}
+
+// The Hermite -> Cartesian transform of the uniform-ket kernel as a roofline probe: per iteration 20 lane-private LDS.64 from a
+// conflict-free shared-memory column (element e of lane x at R[e * 32 + x], the layout of the R tensor) feed 20 independent
+// DFMAs, one warp per block, `warps_per_sm` resident warps.  The rate it reaches is the shared-memory ceiling of that transform.
+__global__ void __launch_bounds__(32) lds_dfma_probe_kernel(double* out, int iters, double e) {
+    extern __shared__ double sm[];
+    double* R = sm + threadIdx.x;
+    for (int i = 0; i < 192; ++i) R[i * 32] = i * 0.001 + threadIdx.x;
+    double y[20];
+#pragma unroll
+    for (int i = 0; i < 20; ++i) y[i] = 0.0;
+    for (int it = 0; it < iters; ++it) {
+        const double* Rq = R + (it & 7) * (20 * 32);
+#pragma unroll
+        for (int i = 0; i < 20; ++i) y[i] = fma(e, Rq[i * 32], y[i]);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 20; ++i) s += y[i];
+    out[blockIdx.x * 32 + threadIdx.x] = s;
+}
+
+extern "C" int te_measure_smem_dfma_rate(int warps_per_sm, double* tflops) {
+    if (!tflops || warps_per_sm < 1 || warps_per_sm > 32) { set_error("te_measure_smem_dfma_rate: bad argument"); return TE_ERR_BAD_ARG; }
+    int dev = 0, sms = 0;
+    TE_CUDA(cudaGetDevice(&dev));
+    TE_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int blocks = sms * warps_per_sm, iters = 20000;
+    double* d = nullptr;
+    TE_CUDA(cudaMalloc(&d, (size_t)blocks * 32 * sizeof(double)));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(e0);
+        lds_dfma_probe_kernel<<<blocks, 32, 192 * 32 * sizeof(double)>>>(d, iters, 1.0000001);
+        cudaEventRecord(e1);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0) best = std::max(best, 2.0 * 20 * (double)iters * blocks * 32 / (ms * 1e-3) / 1e12);
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
     TE_CUDA(cudaGetLastError());

@@ -28,6 +28,20 @@ __host__ __device__ constexpr int cart_y(int l, int i) { return cart_row(i) - ca
 // class index of a primitive shell pair, la <= lb: SS SP SD SF PP PD PF DD DF FF
 __host__ __device__ constexpr int pair_class(int la, int lb) { return (la == 0 ? 0 : la == 1 ? 4 : la == 2 ? 7 : 9) + (lb - la); }
 
+// Classes that have an FP32 leg in the mixed-precision build (te_build_jk_mixed): the FP32 kernel is the uniform-ket kernel, so
+// only classes it serves well take part (measured on config 5): not the lightest ones (L <= 2: no FP32 kernel), not the
+// block-per-lane classes (their FP64 kernel is faster than the FP32 uniform-ket kernel) and not the heaviest bras.
+__host__ __device__ constexpr bool jk_fp32_class(int la, int lb, int lc, int ld) {
+    const int L = la + lb + lc + ld;
+    const int outs = ncart(la) * ncart(lb) + (ncart(la) + ncart(lb)) * (ncart(lc) + ncart(ld));
+    if (L <= 2) return false;
+    if (L <= 4 && outs <= 48) return false;
+    if (la + lb >= 5) return false;
+    if (la == 2 && lb == 2 && lc + ld >= 5) return false;
+    if (la == 1 && lb == 3 && lc == 3 && ld == 3) return false;
+    return true;
+}
+
 // ------------------------------------------------------------------------------------------ Boys table
 // F_m(T_i) on the grid T_i = i * BOYS_DT, i = 0..BOYS_NPTS-1, m = 0..BOYS_MROWS-1; used for T < BOYS_TMAX.
 constexpr double BOYS_DT = 1.0 / 16.0;
@@ -35,17 +49,20 @@ constexpr double BOYS_TMAX = 36.0;
 constexpr int BOYS_NPTS = 577;                 // 36 * 16 + 1
 constexpr int BOYS_NTAYLOR = 8;                // terms k = 0..7
 constexpr int BOYS_MROWS = 12 + BOYS_NTAYLOR;  // m = 0..19
+constexpr int BOYS_STRIDE = BOYS_MROWS + 1;    // row of a grid point: F_0..F_19(T_i), then exp(-T_i)
 
 // Boys function F_0..F_L(T) (eq. 18).  T < 36: 8-term Taylor expansion of F_L about the nearest grid point,
 // F_L(T) = sum_k F_{L+k}(T_i) (T_i - T)^k / k!  (truncation < 3e-17 relative), then the stable downward
-// recursion F_{m-1} = (2T F_m + exp(-T)) / (2m-1).  T >= 36: erf(sqrt T) = 1 to double precision, so
-// F_0 = sqrt(pi/T)/2, then upward F_{m+1} = ((2m+1) F_m - exp(-T)) / (2T)  (stable for T >> m).
+// recursion F_{m-1} = (2T F_m + exp(-T)) / (2m-1); exp(-T) = exp(-T_i) exp(T_i - T) with the tabulated exp(-T_i) and an
+// 8-term series in |T_i - T| <= 1/32 (truncation 2e-17 relative), which costs 8 FMAs instead of a libm exp().
+// T >= 36: erf(sqrt T) = 1 to double precision, so F_0 = sqrt(pi/T)/2, then upward
+// F_{m+1} = ((2m+1) F_m - exp(-T)) / (2T)  (stable for T >> m).
 template <int L>
 __device__ __forceinline__ void boys(double T, const double* __restrict__ tab, double* __restrict__ F) {
     if (T < BOYS_TMAX) {
         const int i = __double2int_rn(T * (1.0 / BOYS_DT));
         const double d = (double)i * BOYS_DT - T;
-        const double* row = tab + i * BOYS_MROWS + L;
+        const double* row = tab + i * BOYS_STRIDE + L;
         double s = __ldg(row + 7) * (1.0 / 5040.0);
         s = fma(s, d, __ldg(row + 6) * (1.0 / 720.0));
         s = fma(s, d, __ldg(row + 5) * (1.0 / 120.0));
@@ -56,7 +73,15 @@ __device__ __forceinline__ void boys(double T, const double* __restrict__ tab, d
         s = fma(s, d, __ldg(row + 0));
         F[L] = s;
         if (L > 0) {
-            const double eT = exp(-T), T2 = 2.0 * T;
+            double ed = 1.0 / 5040.0;
+            ed = fma(ed, d, 1.0 / 720.0);
+            ed = fma(ed, d, 1.0 / 120.0);
+            ed = fma(ed, d, 1.0 / 24.0);
+            ed = fma(ed, d, 1.0 / 6.0);
+            ed = fma(ed, d, 0.5);
+            ed = fma(ed, d, 1.0);
+            ed = fma(ed, d, 1.0);
+            const double eT = __ldg(row + (BOYS_MROWS - L)) * ed, T2 = 2.0 * T;
 #pragma unroll
             for (int m = L; m > 0; --m) F[m - 1] = fma(T2, F[m], eT) * (1.0 / (2 * m - 1));
         }
@@ -78,26 +103,41 @@ struct PairD {
     double PB[3];   // P - B
     double p;       // a + b
     double pref;    // c~_m c~_n exp(-ab/p |A-B|^2): eq. 7 prefactors of all three dimensions folded in
+    double rp;      // 1 / p (the quartet prefactor is formed from rp, rq and one rsqrt(p + q), without a division)
 };
+
+// Exponent of the auxiliary integrals and prefactor of a primitive quartet: alpha = pq/(p+q), 2 pi^{5/2} / (p q sqrt(p+q))
+// (eq. 30).  omega2 = omega^2 > 0 selects the long-range operator erf(omega r)/r of eq. 32-33:
+// alpha -> pq omega^2 / (pq + (p+q) omega^2) = alpha omega^2 / (alpha + omega^2) and the prefactor gains omega / sqrt(alpha + omega^2).
+__device__ __forceinline__ void eri_scale(double p, double rp, double q, double rq, double omega2, double& alpha, double& pref) {
+    const double s = rsqrt(p + q);   // 1 / sqrt(p + q)
+    alpha = p * q * (s * s);
+    pref = 34.986836655249725693 * (rp * rq) * s;
+    if (omega2 > 0.0) {
+        const double w = omega2 / (alpha + omega2);
+        alpha *= w;
+        pref *= sqrt(w);
+    }
+}
 
 // E coefficients of one dimension, eq. 5-8 with E^{00}_0 = 1 (the eq. 7 exponential lives in PairD::pref).
 // E[i][j][t], zero for t > i+j.  SIGN: multiply by (-1)^t (the ket factor of eq. 30).
-template <int LA, int LB, bool SIGN>
-__device__ __forceinline__ void etable(double PA, double PB, double h, double (&E)[LA + 1][LB + 1][LA + LB + 1]) {
+template <int LA, int LB, bool SIGN, class T>
+__device__ __forceinline__ void etable(T PA, T PB, T h, T (&E)[LA + 1][LB + 1][LA + LB + 1]) {
 #pragma unroll
     for (int i = 0; i <= LA; ++i)
 #pragma unroll
         for (int j = 0; j <= LB; ++j)
 #pragma unroll
-            for (int t = 0; t <= LA + LB; ++t) E[i][j][t] = 0.0;
-    E[0][0][0] = 1.0;
+            for (int t = 0; t <= LA + LB; ++t) E[i][j][t] = T(0);
+    E[0][0][0] = T(1);
 #pragma unroll
     for (int i = 0; i < LA; ++i)
 #pragma unroll
         for (int t = 0; t <= i + 1; ++t) {
-            double v = PA * E[i][0][t];
+            T v = PA * E[i][0][t];
             if (t > 0) v = fma(h, E[i][0][t - 1], v);
-            if (t + 1 <= i) v = fma((double)(t + 1), E[i][0][t + 1], v);
+            if (t + 1 <= i) v = fma(T(t + 1), E[i][0][t + 1], v);
             E[i + 1][0][t] = v;
         }
 #pragma unroll
@@ -106,9 +146,9 @@ __device__ __forceinline__ void etable(double PA, double PB, double h, double (&
         for (int j = 0; j < LB; ++j)
 #pragma unroll
             for (int t = 0; t <= i + j + 1; ++t) {
-                double v = PB * E[i][j][t];
+                T v = PB * E[i][j][t];
                 if (t > 0) v = fma(h, E[i][j][t - 1], v);
-                if (t + 1 <= i + j) v = fma((double)(t + 1), E[i][j][t + 1], v);
+                if (t + 1 <= i + j) v = fma(T(t + 1), E[i][j][t + 1], v);
                 E[i][j + 1][t] = v;
             }
     if (SIGN) {
@@ -167,19 +207,19 @@ __device__ __forceinline__ void rtable(double alpha, double X, double Y, double 
 // FULL = fully unrolled (all indices compile-time, arrays in registers); otherwise rolled loops.
 template <int LA, int LB, int LC, int LD, bool FULL, class Emit>
 __device__ __forceinline__ void md_quartet(const PairD& bra, const PairD& ket, const double* __restrict__ boys_tab,
-                                           Emit& emit) {
+                                           Emit& emit, double omega2 = 0.0) {
     constexpr int LAB = LA + LB, LCD = LC + LD, L = LAB + LCD;
     constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
     constexpr int UN = FULL ? 64 : 1;
-    const double p = bra.p, q = ket.p, pq = p + q;
-    const double alpha = p * q / pq;
+    const double p = bra.p, q = ket.p;
+    double alpha, pref;
+    eri_scale(p, bra.rp, q, ket.rp, omega2, alpha, pref);
     const double X = bra.P[0] - ket.P[0], Y = bra.P[1] - ket.P[1], Z = bra.P[2] - ket.P[2];
     double F[L + 1];
     boys<L>(alpha * (X * X + Y * Y + Z * Z), boys_tab, F);
     double R[nherm(L)];
     rtable<L>(alpha, X, Y, Z, F, R);
-    // 2 pi^{5/2} / (p q sqrt(p+q)) (eq. 30) times both pair prefactors
-    const double pref = 34.986836655249725693 / (p * q * sqrt(pq)) * bra.pref * ket.pref;
+    pref *= bra.pref * ket.pref;   // eq. 30 prefactor times both pair prefactors
 
     double Eb[3][LA + 1][LB + 1][LAB + 1], Ek[3][LC + 1][LD + 1][LCD + 1];
     {
