@@ -44,6 +44,7 @@ extern "C" {
 #define TE_ERR_CUDA (-4)
 
 #define TE_NCLASS 10 /* primitive shell-pair classes SS SP SD SF PP PD PF DD DF FF */
+#define TE_NOALLOC_MAX_NBF 512 /* largest nbf te_nuclear_attraction_noalloc accepts: 512^2 doubles = 2 MiB of static device scratch */
 
 typedef struct te_basis te_basis; /* opaque */
 typedef struct te_pairs te_pairs; /* opaque */
@@ -134,6 +135,16 @@ int te_jk_stats(const te_pairs *p, long long quartets[TE_NCLASS][TE_NCLASS], flo
  * slots of the warp batches that ran the integral code, so live / slots is the lane occupancy of the class kernel.
  * Either pointer may be NULL. */
 int te_jk_screening_stats(const te_pairs *p, long long visited[TE_NCLASS][TE_NCLASS], long long slots[TE_NCLASS][TE_NCLASS]);
+/* The same matrix for callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc):
+ * this call performs NO allocation, on the host or on the device (no cudaMalloc / cudaFree, no allocating library routine) and
+ * no synchronisation; it is asynchronous on cuda_stream.  Its nbf x nbf accumulator is a file-scope static device array of
+ * TE_NOALLOC_MAX_NBF^2 doubles (2 MiB, held by every GPU that loads the library until the process exits), so
+ * nbf > TE_NOALLOC_MAX_NBF is rejected with TE_ERR_BAD_ARG (use te_nuclear_attraction).  The charges are a DEVICE array
+ * xyzq_dev[ncharge][4] = (x, y, z, q_C), caller-owned, 8-byte aligned.  V_dev: DEVICE nbf x nbf, OVERWRITTEN.  Every call on a
+ * device shares the one array: calls that overlap on the GPU (different streams, or different handles) RACE -- serialise them.
+ * The array keeps the last call's contents; each call clears what it uses before accumulating.  Does not touch the handle's
+ * scratch, so it may overlap a J/K build on the same handle. */
+int te_nuclear_attraction_noalloc(const te_pairs *p, int ncharge, const double *xyzq_dev, double *V_dev, void *cuda_stream);
 /* Kernel family used by the builds on this handle: 2 (default) = the measured per-class choice; 0 = generic
  * thread-per-quartet kernel for every class, 1 = uniform-ket warp kernel wherever it exists, 3 = split-quartet kernel
  * wherever it exists.  Every family computes the same J and K (tests hold each to the parity bar). */

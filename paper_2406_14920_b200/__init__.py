@@ -66,6 +66,7 @@ def lib():
     L.te_build_j.argtypes = [vp, vp, vp, C.c_double, vp]
     L.te_jk_precision_stats.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
     L.te_nuclear_attraction.argtypes = [vp, C.c_int, dpp, dpp, vp, vp]
+    L.te_nuclear_attraction_noalloc.argtypes = [vp, C.c_int, vp, vp, vp]
     L.te_jk_set_kernel_family.argtypes = [vp, C.c_int]
     L.te_measure_smem_dfma_rate.argtypes = [C.c_int, dpp]
     L.te_jk_stats.argtypes = [vp, C.POINTER(C.c_longlong), C.POINTER(C.c_float)]
@@ -226,6 +227,19 @@ class Pairs:
         st = stream if stream is not None else torch.cuda.current_stream()
         _check(lib().te_nuclear_attraction(self.handle, int(q_c.shape[0]), _dp(xyz_c), _dp(q_c), C.c_void_p(V.data_ptr()),
                                            C.c_void_p(st.cuda_stream)), "te_nuclear_attraction")
+        return V
+
+    def nuclear_attraction_noalloc(self, xyzq, V, stream=None):
+        """te_nuclear_attraction_noalloc: charges xyzq[n, 4] and output V[nbf, nbf] are caller-owned torch CUDA float64
+        tensors; the call allocates nothing (nbf <= TE_NOALLOC_MAX_NBF = 512) and is asynchronous on `stream`."""
+        import torch
+        n = self.basis.nbf
+        assert xyzq.is_cuda and xyzq.dtype == torch.float64 and xyzq.is_contiguous() and xyzq.dim() == 2 and xyzq.shape[1] == 4
+        assert V.is_cuda and V.dtype == torch.float64 and V.is_contiguous() and tuple(V.shape) == (n, n)
+        st = stream if stream is not None else torch.cuda.current_stream()
+        _check(lib().te_nuclear_attraction_noalloc(self.handle, int(xyzq.shape[0]), C.c_void_p(xyzq.data_ptr()),
+                                                   C.c_void_p(V.data_ptr()), C.c_void_p(st.cuda_stream)),
+               "te_nuclear_attraction_noalloc")
         return V
 
     def set_kernel_family(self, family: int):

@@ -46,7 +46,9 @@ def build(force: bool = False, jobs: int | None = None) -> str:
     """Compile what is stale (an object is stale when one of ITS sources is newer) and link."""
     os.makedirs(BUILD, exist_ok=True)
     work = [(os.path.join(CSRC, "te_lib.cu"), os.path.join(BUILD, "te_lib.o"), [], _newest(["te_lib.cu"] + _COMMON)),
-            (os.path.join(CSRC, "te_dispatch.cu"), os.path.join(BUILD, "te_dispatch.o"), [], _newest(["te_dispatch.cu"] + _COMMON))]
+            (os.path.join(CSRC, "te_dispatch.cu"), os.path.join(BUILD, "te_dispatch.o"), [], _newest(["te_dispatch.cu"] + _COMMON)),
+            (os.path.join(CSRC, "te_noalloc.cu"), os.path.join(BUILD, "te_noalloc.o"), [],
+             _newest(["te_noalloc.cu", "te_kernels.cuh"] + _COMMON))]
     inst_dep = _newest(["te_inst.cu"] + _COMMON + _KERNELS)
     # slowest translation units first so the pool stays busy
     for cb in (4, 2, 3, 5, 6, 7, 9, 8, 0, 1):
