@@ -46,7 +46,7 @@ int TE_CAT(launch_pair_fill_cb, TE_CB)(const te_basis* b, long long n, const lon
 // uniform-ket kernel in precision T: one warp per block, per-lane R tensor in shared memory
 template <class T, int LC, int LD>
 static int launch_w(te_pairs* P, JKArgs& a, double tau, int lane, int dev, int sms, cudaStream_t st) {
-    using S = WShape<LA, LB, LC, LD>;
+    using S = WShape<LA, LB, LC, LD, T>;
     constexpr int smem = S::smem_doubles * (int)sizeof(T);
     static int bps[TE_MAX_DEV] = {0};
     std::lock_guard<std::mutex> lock(g_cache_mutex);

@@ -130,19 +130,19 @@ __global__ void __launch_bounds__(WARP) jkb_kernel(JKArgs a) {
                 }
                 if (fl & 2) {
 #pragma unroll
-                    for (int x = 0; x < NA * NC; ++x) atomicAdd(&a.Kt[(offA + x / NC) * nbf + ik.offA + x % NC], kac[x]);
+                    for (int x = 0; x < NA * NC; ++x) atomicAdd(&a.Kt[(ik.offA + x % NC) * nbf + offA + x / NC], kac[x]);
                 }
                 if (fl & 4) {
 #pragma unroll
-                    for (int x = 0; x < NB * NC; ++x) atomicAdd(&a.Kt[(offB + x / NC) * nbf + ik.offA + x % NC], kbc[x]);
+                    for (int x = 0; x < NB * NC; ++x) atomicAdd(&a.Kt[(ik.offA + x % NC) * nbf + offB + x / NC], kbc[x]);
                 }
                 if (fl & 8) {
 #pragma unroll
-                    for (int x = 0; x < NA * ND; ++x) atomicAdd(&a.Kt[(offA + x / ND) * nbf + ik.offB + x % ND], kad[x]);
+                    for (int x = 0; x < NA * ND; ++x) atomicAdd(&a.Kt[(ik.offB + x % ND) * nbf + offA + x / ND], kad[x]);
                 }
                 if (fl & 16) {
 #pragma unroll
-                    for (int x = 0; x < NB * ND; ++x) atomicAdd(&a.Kt[(offB + x / ND) * nbf + ik.offB + x % ND], kbd[x]);
+                    for (int x = 0; x < NB * ND; ++x) atomicAdd(&a.Kt[(ik.offB + x % ND) * nbf + offB + x / ND], kbd[x]);
                 }
                 assigned = false;
             }
@@ -162,23 +162,27 @@ __global__ void __launch_bounds__(WARP) jkb_kernel(JKArgs a) {
                     dm_kad = a.Dm[ib.shB * ns + ik.shA];
                     dm_kbd = a.Dm[ib.shA * ns + ik.shA];
                     mjab = 1.0;
+                    // D is symmetric (te_jk.h), and K = Kt + Kt^T is formed at the end: every bra-ket density element is read, and every K
+                    // contribution added, at [ket AO row][bra AO column].  The ket is uniform across the warp, so the lanes of a warp
+                    // (and all warps on the same ket) touch a handful of rows instead of rows scattered over the whole matrix.
                     const double* Da = a.Ds + (long long)offA * nbf;
-                    const double* Db = a.Ds + (long long)offB * nbf;
+                    const double* Dc = a.Ds + (long long)ik.offA * nbf;
+                    const double* Dd = a.Ds + (long long)ik.offB * nbf;
 #pragma unroll
                     for (int i = 0; i < NA; ++i) {
 #pragma unroll
                         for (int jj = 0; jj < NB; ++jj) { dab[i * NB + jj] = Da[i * nbf + offB + jj]; jab[i * NB + jj] = 0.0; }
 #pragma unroll
-                        for (int l = 0; l < ND; ++l) { dal[i * ND + l] = Da[i * nbf + ik.offB + l]; kad[i * ND + l] = 0.0; }
+                        for (int l = 0; l < ND; ++l) { dal[i * ND + l] = Dd[l * nbf + offA + i]; kad[i * ND + l] = 0.0; }
 #pragma unroll
-                        for (int k = 0; k < NC; ++k) { dak[i * NC + k] = Da[i * nbf + ik.offA + k]; kac[i * NC + k] = 0.0; }
+                        for (int k = 0; k < NC; ++k) { dak[i * NC + k] = Dc[k * nbf + offA + i]; kac[i * NC + k] = 0.0; }
                     }
 #pragma unroll
                     for (int jj = 0; jj < NB; ++jj) {
 #pragma unroll
-                        for (int l = 0; l < ND; ++l) { dbl[jj * ND + l] = Db[jj * nbf + ik.offB + l]; kbd[jj * ND + l] = 0.0; }
+                        for (int l = 0; l < ND; ++l) { dbl[jj * ND + l] = Dd[l * nbf + offB + jj]; kbd[jj * ND + l] = 0.0; }
 #pragma unroll
-                        for (int k = 0; k < NC; ++k) { dbk[jj * NC + k] = Db[jj * nbf + ik.offA + k]; kbc[jj * NC + k] = 0.0; }
+                        for (int k = 0; k < NC; ++k) { dbk[jj * NC + k] = Dc[k * nbf + offB + jj]; kbc[jj * NC + k] = 0.0; }
                     }
                 } else {
                     cur = 0; end = 0;

@@ -38,7 +38,10 @@ static __constant__ RowTab c_rowtab = RowTab();
 
 constexpr int WARP = 32;
 
-template <int LA, int LB, int LC, int LD>
+#ifndef TE_KBAT
+#define TE_KBAT 1
+#endif
+template <int LA, int LB, int LC, int LD, class T = double>
 struct WShape {
     static constexpr int LAB = LA + LB, LCD = LC + LD, L = LAB + LCD;
     static constexpr int NA = ncart(LA), NB = ncart(LB), NC = ncart(LC), ND = ncart(LD);
@@ -57,14 +60,24 @@ struct WShape {
     // (t',u') and a run-time v' loop -- except against pd-sized kets (LCD <= 3), where compile-time v' also wins ((PD|PD)
     // 351 -> 281 ms); for larger kets it gains < 2 % and triples the compile time of the library.
     static constexpr int SIZE = NHB * NNZK + nnz_e(LA, LB) * NC * ND;
-    static constexpr int VAR = LCD == 6 ? 1   // ff kets (FP32 leg / forced family only): the 84-entry compile-time box costs minutes of ptxas
+    // k-batched form (VAR 3, below): FP64 only, s / sp bras against kets up to df, sd / pp bras against kets up to LCD = 4 (for df
+    // kets the 20 ket_batch instantiations per class cost 30 minutes of compile time per translation unit for a 20 % gain)
+    static constexpr bool KBEL = TE_KBAT && sizeof(T) == 8 && NC >= 3 && (NHB <= 4 ? LCD <= 5 : (NHB <= 10 && LCD <= 4));
+    static constexpr int VAR = KBEL ? 3
+                             : LCD == 6 ? 1   // ff kets (FP32 leg / forced family only): the 84-entry compile-time box costs minutes of ptxas
                              : (LA == 1 && LB == 1) ? 2
                              : NHB <= 10 ? (SIZE <= 6000 ? 0 : 2)
                              : (LA == 0 && LB == 3 && LC == 0 && LD == 3) ? 0 : (LCD <= 3 ? 2 : 1);
     static constexpr bool UNR = VAR == 0;
     static constexpr bool V2CT = VAR == 2;
+    // VAR 3, "k-batched" ket transform (light bras, NHB <= 10, kets up to df): for a fixed l the Hermite boxes of the ket components k
+    // overlap, so one R element loaded from the lane's shared-memory column feeds the FMAs of every k of a batch whose box holds
+    // that shift Q (1.6-3 FMAs per private load instead of 1), all offsets compile-time (ket_batch below).
+    static constexpr bool KBAT = VAR == 3;
+    static constexpr int KBN = !KBAT ? 1 : (NC * NHB <= 32 ? NC : (NC % 3 == 0 ? 3 : (NC % 2 == 0 ? 2 : 1)));   // components per batch
+    static constexpr int NKB = NC / KBN;
     static constexpr int UNK = UNR ? 128 : 1;
-    static constexpr bool KEEPC = UNR && (NA + NB) * NC <= 24;
+    static constexpr bool KEEPC = (UNR || KBAT) && (NA + NB) * NC <= 24;
     // NL = lanes of the warp that hold a quartet (R column stride).  Measured on B200: narrowing the warp to 8 lanes for L >= 10
     // (4x more resident warps) made (DF|DF) 2.4x SLOWER -- these kernels are bound by per-warp instruction / local-memory
     // throughput, not by latency -- so every lane holds a quartet.
@@ -100,6 +113,76 @@ __device__ __forceinline__ void flush_vec(bool runs, int maxdist, int dist, bool
 #pragma unroll
         for (int x = 0; x < N; ++x) atomicAdd(addr(x), (double)v[x]);
     }
+}
+
+// Offset of the E~ entries of the ket component pair (k,l) in the kt table (built in loop order l, k, t', u', v').
+template <int LC, int LD>
+__host__ __device__ constexpr int kt_off(int l, int k) {
+    int s = 0;
+    for (int l2 = 0; l2 < ncart(LD); ++l2)
+        for (int k2 = 0; k2 < ncart(LC); ++k2) {
+            if (l2 == l && k2 == k) return s;
+            s += (cart_x(LC, k2) + cart_x(LD, l2) + 1) * (cart_y(LC, k2) + cart_y(LD, l2) + 1) * (cart_z(LC, k2) + cart_z(LD, l2) + 1);
+        }
+    return s;
+}
+// largest power of component k in [K0, K0 + KN) along dimension d (0 x, 1 y, 2 z)
+template <int LC>
+__host__ __device__ constexpr int kmax_pow(int K0, int KN, int d) {
+    int m = 0;
+    for (int k = K0; k < K0 + KN; ++k) {
+        const int v = d == 0 ? cart_x(LC, k) : (d == 1 ? cart_y(LC, k) : cart_z(LC, k));
+        m = v > m ? v : m;
+    }
+    return m;
+}
+template <int LC, int LD>
+__host__ __device__ constexpr bool in_box(int k, int l, int t2, int u2, int v2) {
+    return t2 <= cart_x(LC, k) + cart_x(LD, l) && u2 <= cart_y(LC, k) + cart_y(LD, l) && v2 <= cart_z(LC, k) + cart_z(LD, l);
+}
+template <int LC, int LD>
+__host__ __device__ constexpr bool in_any_box(int K0, int KN, int l, int t2, int u2, int v2) {
+    for (int k = K0; k < K0 + KN; ++k)
+        if (in_box<LC, LD>(k, l, t2, u2, v2)) return true;
+    return false;
+}
+
+// Ket Hermite -> Cartesian for the components k = K0 .. K0+KN-1 at fixed l:  Y[kk][P] = sum_{Q in box(k,l)} E~_Q^{kl} R_{P+Q}.
+// Walks the UNION of the boxes once; an R element is loaded once per shift Q and used by every k whose box holds Q.
+template <class T, int LAB, int LC, int LD, int NL, int l, int K0, int KN>
+__device__ __forceinline__ void ket_batch(const T* __restrict__ Rl, const T* __restrict__ kt, T (&Y)[KN * nherm(LAB)]) {
+    constexpr int LCD = LC + LD, L = LAB + LCD, NHB = nherm(LAB);
+    constexpr int lx = cart_x(LD, l), ly = cart_y(LD, l), lz = cart_z(LD, l);
+    constexpr int MX = lx + kmax_pow<LC>(K0, KN, 0), MY = ly + kmax_pow<LC>(K0, KN, 1), MZ = lz + kmax_pow<LC>(K0, KN, 2);
+#pragma unroll
+    for (int x = 0; x < KN * NHB; ++x) Y[x] = T(0);
+    static_for<MX + 1>([&](auto T2) {
+        constexpr int t2 = decltype(T2)::value;
+        static_for<MY + 1>([&](auto U2) {
+            constexpr int u2 = decltype(U2)::value;
+            static_for<MZ + 1>([&](auto V2) {
+                constexpr int v2 = decltype(V2)::value;
+                if constexpr (in_any_box<LC, LD>(K0, KN, l, t2, u2, v2)) {
+                    T r[NHB];
+#pragma unroll
+                    for (int t = 0; t <= LAB; ++t)
+#pragma unroll
+                        for (int u = 0; u <= LAB - t; ++u)
+#pragma unroll
+                            for (int v = 0; v <= LAB - t - u; ++v) r[tidx<LAB>(t, u, v)] = Rl[(tidx<L>(t + t2, u + u2, 0) + v + v2) * NL];
+                    static_for<KN>([&](auto KKc) {
+                        constexpr int kk = decltype(KKc)::value, k = K0 + kk;
+                        if constexpr (in_box<LC, LD>(k, l, t2, u2, v2)) {
+                            constexpr int sy = cart_y(LC, k) + ly, sz = cart_z(LC, k) + lz;
+                            const T e = kt[kt_off<LC, LD>(l, k) + (t2 * (sy + 1) + u2) * (sz + 1) + v2];
+#pragma unroll
+                            for (int P = 0; P < NHB; ++P) Y[kk * NHB + P] = fma(e, r[P], Y[kk * NHB + P]);
+                        }
+                    });
+                }
+            });
+        });
+    });
 }
 
 // R^0_{tuv} of eq. 21-25 built in place in a shared-memory column (element i at R[i * 32]); same sweep as rtable<L>.
@@ -143,7 +226,7 @@ __device__ __forceinline__ void rtable_sm(T alpha, T X, T Y, T Z, const T* __res
 // sums are added to the FP64 J / K accumulators.
 template <class T, int LA, int LB, int LC, int LD>
 __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
-    using S = WShape<LA, LB, LC, LD>;
+    using S = WShape<LA, LB, LC, LD, T>;
     constexpr int LAB = S::LAB, LCD = S::LCD, L = S::L;
     constexpr int NA = S::NA, NB = S::NB, NC = S::NC, ND = S::ND, NHB = S::NHB;
     constexpr bool KEEPC = S::KEEPC;
@@ -270,7 +353,11 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
 #pragma unroll
                 for (int x = 0; x < S::NKC; ++x) kcl[x * NL] = 0.0;
             }
-            const double* Da = nullptr; const double* Db = nullptr;   // rows of the scaled density at the bra's AOs
+            // D is symmetric and K = Kt + Kt^T is formed at the end: bra-ket density elements are read, and K contributions added, at
+            // [ket AO row][bra AO column] -- the ket is warp-uniform, so a warp touches a few rows instead of scattered ones
+            const double* Da = nullptr;                                     // rows of the scaled density at the bra's first shell (D_ab)
+            const double* const Dc = a.Ds + (long long)ik.offA * nbf;       // rows at the ket's AOs
+            const double* const Dd = a.Ds + (long long)ik.offB * nbf;
             if (active) {
                 ++nlive;
                 bp = a.pb[bi];
@@ -296,7 +383,6 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                 etable<LA, LB, false>((T)bp.PA[1], (T)bp.PB[1], hb, Eby);
                 etable<LA, LB, false>((T)bp.PA[2], (T)bp.PB[2], hb, Ebz);
                 Da = a.Ds + (long long)ib.offA * nbf;
-                Db = a.Ds + (long long)ib.offB * nbf;
 #pragma unroll
                 for (int i = 0; i < NA; ++i)
 #pragma unroll
@@ -305,9 +391,9 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
 #pragma unroll
                     for (int k = 0; k < NC; ++k) {
 #pragma unroll
-                        for (int i = 0; i < NA; ++i) dac[i * NC + k] = (T)Da[i * nbf + ik.offA + k];
+                        for (int i = 0; i < NA; ++i) dac[i * NC + k] = (T)Dc[k * nbf + ib.offA + i];
 #pragma unroll
-                        for (int jj = 0; jj < NB; ++jj) dbc[jj * NC + k] = (T)Db[jj * nbf + ik.offA + k];
+                        for (int jj = 0; jj < NB; ++jj) dbc[jj * NC + k] = (T)Dc[k * nbf + ib.offB + jj];
                     }
                 }
             }
@@ -322,12 +408,14 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                 for (int jj = 0; jj < NB; ++jj) kbl[jj] = 0.0;
                 if (active) {
 #pragma unroll
-                    for (int i = 0; i < NA; ++i) dal[i] = Da[i * nbf + ik.offB + l];
+                    for (int i = 0; i < NA; ++i) dal[i] = Dd[l * nbf + ib.offA + i];
 #pragma unroll
-                    for (int jj = 0; jj < NB; ++jj) dbl[jj] = Db[jj * nbf + ik.offB + l];
+                    for (int jj = 0; jj < NB; ++jj) dbl[jj] = Dd[l * nbf + ib.offB + jj];
                 }
-#pragma unroll UNK
-                for (int k = 0; k < NC; ++k) {
+                T Yall[S::KBAT ? S::KBN * NHB : 1];
+                // always_inline: called from NC sites in the k-batched form; an out-of-line lambda would push every captured array to the stack
+                auto kbody = [&](const int k, auto KK) __attribute__((always_inline)) {   // KK: position of k in Yall (k-batched), -1 otherwise
+                    constexpr int kk = decltype(KK)::value;
                     const int sx = cart_x(LC, k) + lx, sy = cart_y(LC, k) + ly, sz = cart_z(LC, k) + lz;
                     T jkl = 0.0;
                     T kak[KEEPC ? 1 : NA], kbk[KEEPC ? 1 : NB];
@@ -343,7 +431,10 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
 #pragma unroll
                         for (int P = 0; P < NHB; ++P) Yv[P] = 0.0;
                         const T* ktp = kt + ptr;
-                        if constexpr (UNR) {
+                        if constexpr (kk >= 0) {
+#pragma unroll
+                            for (int P = 0; P < NHB; ++P) Yv[P] = Yall[(kk >= 0 ? kk : 0) * NHB + P];
+                        } else if constexpr (UNR) {
 #pragma unroll
                             for (int t2 = 0; t2 <= sx; ++t2)
 #pragma unroll
@@ -405,9 +496,9 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                         T dbk[KEEPC ? 1 : NB], dak[KEEPC ? 1 : NA];
                         if (!KEEPC) {
 #pragma unroll
-                            for (int i = 0; i < NA; ++i) dak[i] = Da[i * nbf + ik.offA + k];
+                            for (int i = 0; i < NA; ++i) dak[i] = Dc[k * nbf + ib.offA + i];
 #pragma unroll
-                            for (int jj = 0; jj < NB; ++jj) dbk[jj] = Db[jj * nbf + ik.offA + k];
+                            for (int jj = 0; jj < NB; ++jj) dbk[jj] = Dc[k * nbf + ib.offB + jj];
                         }
                         const T dkl = dcd[k * ND + l];
 #pragma unroll
@@ -459,16 +550,30 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
                         for (int o = 16; o > 0; o >>= 1) jkl += __shfl_xor_sync(FULLMASK, jkl, o);
                         if (lane == 0) atomicAdd(&a.Jt[(ik.offA + k) * nbf + ik.offB + l], 2.0 * jkl);
                     }
+                };
+                if constexpr (S::KBAT) {
+                    static_for<S::NKB>([&](auto KBc) __attribute__((always_inline)) {
+                        constexpr int kb = decltype(KBc)::value;
+                        if (active) {
+                            static_for<ND>([&](auto Lc) {
+                                if (l == decltype(Lc)::value) ket_batch<T, LAB, LC, LD, NL, decltype(Lc)::value, kb * S::KBN, S::KBN>(Rl, kt, Yall);
+                            });
+                        }
+                        static_for<S::KBN>([&](auto KK) __attribute__((always_inline)) { kbody(kb * S::KBN + decltype(KK)::value, KK); });
+                    });
+                } else {
+#pragma unroll UNK
+                    for (int k = 0; k < NC; ++k) kbody(k, std::integral_constant<int, -1>{});
                 }
-                flush_vec<NA>(runs, maxdist, dist, head, live_kad, kal, [&](int i) { return &a.Kt[(ib.offA + i) * nbf + ik.offB + l]; });
-                flush_vec<NB>(runs, maxdist, dist, head, live_kbd, kbl, [&](int jj) { return &a.Kt[(ib.offB + jj) * nbf + ik.offB + l]; });
+                flush_vec<NA>(runs, maxdist, dist, head, live_kad, kal, [&](int i) { return &a.Kt[(ik.offB + l) * nbf + ib.offA + i]; });
+                flush_vec<NB>(runs, maxdist, dist, head, live_kbd, kbl, [&](int jj) { return &a.Kt[(ik.offB + l) * nbf + ib.offB + jj]; });
             }
 #pragma unroll
             for (int x = 0; x < NA * NB; ++x) jab[x] *= 2.0;
             flush_vec<NA * NB>(runs, maxdist, dist, head, live_jab, jab, [&](int x) { return &a.Jt[(ib.offA + x / NB) * nbf + ib.offB + x % NB]; });
             if (KEEPC) {
-                flush_vec<(KEEPC ? NA * NC : 1)>(runs, maxdist, dist, head, live_kac, kac, [&](int x) { return &a.Kt[(ib.offA + x / NC) * nbf + ik.offA + x % NC]; });
-                flush_vec<(KEEPC ? NB * NC : 1)>(runs, maxdist, dist, head, live_kbc, kbc, [&](int x) { return &a.Kt[(ib.offB + x / NC) * nbf + ik.offA + x % NC]; });
+                flush_vec<(KEEPC ? NA * NC : 1)>(runs, maxdist, dist, head, live_kac, kac, [&](int x) { return &a.Kt[(ik.offA + x % NC) * nbf + ib.offA + x / NC]; });
+                flush_vec<(KEEPC ? NB * NC : 1)>(runs, maxdist, dist, head, live_kbc, kbc, [&](int x) { return &a.Kt[(ik.offA + x % NC) * nbf + ib.offB + x / NC]; });
             } else {
                 // the quartet's K_ac / K_bc sums come back from the shared-memory column, NC values (one row of the block) at a time
 #pragma unroll 1
@@ -477,7 +582,7 @@ __global__ void __launch_bounds__(WARP) jkw_kernel(JKArgs a) {
 #pragma unroll
                     for (int k = 0; k < NC; ++k) row[k] = kcl[(r * NC + k) * NL];
                     const long long o1 = (r < NA ? ib.offA + r : ib.offB + (r - NA));
-                    flush_vec<NC>(runs, maxdist, dist, head, r < NA ? live_kac : live_kbc, row, [&](int k) { return &a.Kt[o1 * nbf + ik.offA + k]; });
+                    flush_vec<NC>(runs, maxdist, dist, head, r < NA ? live_kac : live_kbc, row, [&](int k) { return &a.Kt[(ik.offA + k) * nbf + o1]; });
                 }
             }
             __syncwarp();

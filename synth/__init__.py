@@ -4,4 +4,4 @@ This package is the ONLY code shared by the CPU oracle (`oracle/`) and the CUDA 
 (`paper_2406_14920_b200/`).  It holds none of the method's arithmetic: no normalisation, no integrals,
 no screening -- only geometry / exponent / coefficient / density draws.
 """
-from .configs import Problem, make_config, subset_atoms, CONFIG_SEED, ncart  # noqa: F401
+from .configs import Problem, make_config, subset_atoms, digest, CONFIG_SEED, ncart  # noqa: F401

@@ -199,6 +199,18 @@ def make_config(n: int) -> Problem:
     raise ValueError("config number must be 1..5")
 
 
+def digest(prob: Problem) -> dict:
+    """SHA-256 of the generated arrays, so that "same inputs" can be checked across machines:
+    `basis` covers geometry, shells, exponents and coefficients (pure functions of the seeded generator); `density`
+    covers D = C C^T, whose last bits also depend on the BLAS that numpy calls for the product."""
+    import hashlib
+    hb, hd = hashlib.sha256(), hashlib.sha256()
+    for a in (prob.xyz, prob.shell_atom, prob.shell_l, prob.shell_nprim, prob.exponents, prob.coefficients):
+        hb.update(np.ascontiguousarray(a).tobytes())
+    hd.update(np.ascontiguousarray(prob.D).tobytes())
+    return {"basis": hb.hexdigest(), "density": hd.hexdigest()}
+
+
 def subset_atoms(prob: Problem, atom_ids, name=None, max_l=None) -> Problem:
     """Cut-down problem: keep only the listed atoms (and optionally shells with l <= max_l); D is the
     matching principal sub-block (still symmetric PSD)."""
