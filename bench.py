@@ -224,8 +224,13 @@ def main_ours(args, rank, world):
     K = torch.empty_like(D)
     flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device="cuda")   # 256 MB > 126 MB L2
 
+    mixed = args.fp32_below is not None      # te_build_jk_mixed instead of the FP64 build: an extra, not the headline
+
     def step():
-        pairs.build_jk(D, J, K, threshold=prob.tau_jk)
+        if mixed:
+            pairs.build_jk(D, J, K, threshold=prob.tau_jk, fp32_below=args.fp32_below)
+        else:
+            pairs.build_jk(D, J, K, threshold=prob.tau_jk)
 
     for _ in range(max(args.warmup, 0)):
         step()
@@ -289,8 +294,9 @@ def main_ours(args, rank, world):
     line = {
         "metric": METRIC, "value": aggregate(live * args.steps, sec, world), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * step_s, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64" if not mixed else "f64/f32 mixed", "data": "synthetic",
         "config": {"workload": CONFIG_NAMES[args.config], "nbf": n, "primitive_pairs_kept": pairs.nkept,
+                   "build": "te_build_jk (FP64)" if not mixed else f"te_build_jk_mixed(fp32_below={args.fp32_below}); e2e is the FP64 host path",
                    "live_quartets_per_build": live, "visited_quartets_per_build": int(visited.sum()),
                    "live_over_visited": live / max(int(visited.sum()), 1), "lane_occupancy": live / max(int(slots.sum()), 1),
                    "thresholds": [prob.tau_pair, prob.tau_jk],
@@ -324,6 +330,8 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--peaks", action="store_true", help="print the measured FP64 ceilings of this GPU and exit")
+    ap.add_argument("--fp32-below", type=float, default=None,
+                    help="time te_build_jk_mixed with this density-weighted switch (the paper uses 1e-5) instead of the FP64 build")
     args = ap.parse_args()
     if args.peaks:
         main_peaks()

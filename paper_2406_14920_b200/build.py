@@ -51,7 +51,7 @@ def build(force: bool = False, jobs: int | None = None) -> str:
              _newest(["te_noalloc.cu", "te_kernels.cuh"] + _COMMON))]
     inst_dep = _newest(["te_inst.cu"] + _COMMON + _KERNELS)
     # slowest translation units first so the pool stays busy
-    for cb in (4, 2, 3, 5, 6, 7, 9, 8, 0, 1):
+    for cb in (1, 4, 2, 0, 3, 5, 6, 7, 9, 8):
         work.append((os.path.join(CSRC, "te_inst.cu"), os.path.join(BUILD, f"te_inst_{cb}.o"), [f"-DTE_CB={cb}"], inst_dep))
     todo = [w[:3] for w in work if force or not os.path.exists(w[1]) or os.path.getmtime(w[1]) < w[3]]
     objs = [w[1] for w in work]

@@ -132,6 +132,8 @@ constexpr int jkq_lanes(int la, int lb, int lc, int ld, int w) {
 constexpr bool jkq_default(int la, int lb, int lc, int ld) {
     // round 2 (after the uniform-ket kernel stopped flushing per (k,l)): (SD|DF), (PP|DF) and (SD|DD) moved to the uniform-ket kernel
     if (lc == 2 && ld == 3 && ((la == 0 && lb == 2) || (la == 1 && lb == 1))) return false;
+    // with the k-batched ket transform the uniform-ket kernel also wins for s / sp bras against ff kets ((SS|FF) 311 -> 135 ms, (SP|FF) 558 -> 413 ms)
+    if (lc == 3 && ld == 3 && la == 0 && lb <= 1) return false;
     return (lc + ld == 6) || (lc == 2 && ld == 3 && la + lb >= 2) || (la + lb >= 4 && lc + ld >= 4) ||
            (la == 1 && lb == 2 && lc + ld >= 4);
 }

@@ -62,7 +62,7 @@ struct WShape {
     static constexpr int SIZE = NHB * NNZK + nnz_e(LA, LB) * NC * ND;
     // k-batched form (VAR 3, below): FP64 only, s / sp bras against kets up to df, sd / pp bras against kets up to LCD = 4 (for df
     // kets the 20 ket_batch instantiations per class cost 30 minutes of compile time per translation unit for a 20 % gain)
-    static constexpr bool KBEL = TE_KBAT && sizeof(T) == 8 && NC >= 3 && (NHB <= 4 ? LCD <= 5 : (NHB <= 10 && LCD <= 4));
+    static constexpr bool KBEL = TE_KBAT && sizeof(T) == 8 && NC >= 3 && (NHB <= 4 ? LCD <= 6 : (NHB <= 10 && LCD <= 4));
     static constexpr int VAR = KBEL ? 3
                              : LCD == 6 ? 1   // ff kets (FP32 leg / forced family only): the 84-entry compile-time box costs minutes of ptxas
                              : (LA == 1 && LB == 1) ? 2
@@ -74,7 +74,7 @@ struct WShape {
     // overlap, so one R element loaded from the lane's shared-memory column feeds the FMAs of every k of a batch whose box holds
     // that shift Q (1.6-3 FMAs per private load instead of 1), all offsets compile-time (ket_batch below).
     static constexpr bool KBAT = VAR == 3;
-    static constexpr int KBN = !KBAT ? 1 : (NC * NHB <= 32 ? NC : (NC % 3 == 0 ? 3 : (NC % 2 == 0 ? 2 : 1)));   // components per batch
+    static constexpr int KBN = !KBAT ? 1 : (NC * NHB <= 32 ? NC : (NC % 5 == 0 && 5 * NHB <= 32 ? 5 : (NC % 3 == 0 ? 3 : (NC % 2 == 0 ? 2 : 1))));   // components per batch
     static constexpr int NKB = NC / KBN;
     static constexpr int UNK = UNR ? 128 : 1;
     static constexpr bool KEEPC = (UNR || KBAT) && (NA + NB) * NC <= 24;
