@@ -82,8 +82,8 @@ int te_pairs_export(const te_pairs *p, int cls, int *shellA, int *shellB, int *p
 int te_pairs_export_geom(const te_pairs *p, int cls, double *P_xyz, double *p_exp, double *prefactor);
 
 /* One J/K build (section 3.4).  D_dev, J_dev, K_dev: DEVICE, row-major nbf x nbf; D must be
- * symmetric; J and K are OVERWRITTEN (not accumulated) and returned symmetric.  threshold = THRECL of
- * eq. 47; 0 means no screening.  A primitive quartet's contribution X <- D_YZ is included iff
+ * symmetric (the kernels read D_xy or D_yx, whichever is closer in memory to what the warp already touches); J and K
+ * are OVERWRITTEN (not accumulated) and returned symmetric.  threshold = THRECL of eq. 47; 0 means no screening.  A primitive quartet's contribution X <- D_YZ is included iff
  * q_bra * q_ket * max|D_YZ block| >= threshold, separately for each of its J and K updates.
  * Asynchronous on cuda_stream (a cudaStream_t, NULL = default stream). */
 int te_build_jk(te_pairs *p, const double *D_dev, double *J_dev, double *K_dev, double threshold,
