@@ -20,6 +20,9 @@ constexpr int jkb_outputs(int la, int lb, int lc, int ld) {
 // in registers (up to 48 outputs a few of them spill, still faster than the shared-memory R column of the uniform-ket kernel;
 // measured: (ss|ss) and (sd|sd) are faster with one primitive quartet per lane)
 constexpr bool use_jkb(int la, int lb, int lc, int ld) {
+    // round 2: (SP|SF) and (SD|PP) (spilling here: 5e9 local-memory instructions per config-5 launch) are 10-17 % faster in the
+    // uniform-ket kernel since its k-batched ket transform and ket-row accesses
+    if ((la == 0 && lb == 1 && lc == 0 && ld == 3) || (la == 0 && lb == 2 && lc == 1 && ld == 1)) return false;
     return la + lb + lc + ld >= 1 && la + lb + lc + ld <= 4 && jkb_outputs(la, lb, lc, ld) <= 48;
 }
 

@@ -134,6 +134,7 @@ constexpr bool jkq_default(int la, int lb, int lc, int ld) {
     if (lc == 2 && ld == 3 && ((la == 0 && lb == 2) || (la == 1 && lb == 1))) return false;
     // with the k-batched ket transform the uniform-ket kernel also wins for s / sp bras against ff kets ((SS|FF) 311 -> 135 ms, (SP|FF) 558 -> 413 ms)
     if (lc == 3 && ld == 3 && la == 0 && lb <= 1) return false;
+    if (la == 0 && lb == 3 && lc == 2 && ld == 3) return false;   // (SF|DF): 497 -> 460 ms in the uniform-ket kernel
     return (lc + ld == 6) || (lc == 2 && ld == 3 && la + lb >= 2) || (la + lb >= 4 && lc + ld >= 4) ||
            (la == 1 && lb == 2 && lc + ld >= 4);
 }
